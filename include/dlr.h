@@ -1,0 +1,126 @@
+/*
+ * dlr.h - C ABI of the B200 (sm_100a, fp64) hot path of the second-order projector-splitting dynamical
+ * low-rank (DLR) integrator for the 6D Vlasov-Poisson equations,
+ *     Cassini & Einkemmer, arXiv 2110.13481 (cited as PAPER.md:<line>), Algorithm 2
+ * with the Fourier-spectral / exponential-integrator sub-steps of section 4.
+ *
+ * State: f(x,v) ~ sum_ij X_i(x) S_ij V_j(v) on a periodic n_x^3 x n_v^3 grid:
+ *   X : N_x x r, column-major (each column = one low-rank factor on the grid),
+ *       grid index I = i1 + n1*(i2 + n2*i3)  (x1 fastest),  h_x^3 X^T X = I
+ *   S : r x r, column-major
+ *   V : N_v x r, column-major, same linearisation, h_v^3 V^T V = I
+ * All numbers are IEEE fp64 ("double precision").  Every step of the path runs in CUDA
+ * kernels of this library; there is no CPU fallback: without a CUDA device every call that touches the
+ * device returns DLR_ERR_CUDA.
+ *
+ * Conventions: C linkage, no exceptions cross the boundary, return 0 = DLR_OK, negative = error.
+ * Pointers are HOST pointers unless the argument is documented as device / "on_device".
+ * One context per stream/thread; no global state.
+ */
+#ifndef DLR_B200_H
+#define DLR_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    DLR_OK = 0,
+    DLR_ERR_INVALID = -1,          /* null pointer / bad argument */
+    DLR_ERR_UNSUPPORTED = -2,      /* grid size or rank outside the supported set */
+    DLR_ERR_WORKSPACE = -3,        /* workspace too small or misaligned */
+    DLR_ERR_CUDA = -4,             /* a CUDA runtime call failed (see dlr_last_cuda_error) */
+    DLR_ERR_NOT_ORTHONORMAL = -5,  /* dlr_set_initial: h^3 X^T X or h^3 V^T V differs from I by > 1e-10 */
+    DLR_ERR_NO_STATE = -6          /* dlr_step / dlr_moments before dlr_set_initial */
+};
+
+/* Grid descriptors of Fig. 2: number of points, left extreme, right extreme of the
+ * periodic box per direction (grid spacing h = (hi-lo)/n, points lo + i*h, i = 0..n-1).
+ * Supported: n_x[0]=n_x[1]=n_x[2] and n_v[0]=n_v[1]=n_v[2], each a power of two in 8..256 (n_x may differ
+ * from n_v); rank in {5, 8, 10, 15, 20}. */
+typedef struct dlr_config {
+    int32_t n_x[3], n_v[3];
+    double x_lo[3], x_hi[3], v_lo[3], v_hi[3];
+    int32_t rank;
+    int32_t order;      /* 2 = Algorithm 2; 1 = Algorithm 1 */
+    double e_scale;     /* multiplies the electric field; 1.0 = the paper's equations, 0.0 = test hook "E = 0" */
+    uint32_t flags;     /* reserved, must be 0 */
+} dlr_config;
+
+/* Diagnostics the paper plots (Figs. 4-7). */
+typedef struct dlr_moments_t {
+    double mass;               /* int int f dx dv          = (h_x^3 1^T X) S (h_v^3 V^T 1)                 */
+    double momentum[3];        /* int int v_i f dx dv                                                      */
+    double kinetic_energy;     /* 1/2 int int |v|^2 f dx dv                                                */
+    double electric_energy;    /* 1/2 int |E|^2 dx, E from eq. (12) + Poisson on the state  */
+    double s_fro;              /* ||S||_F                                                                   */
+    int32_t qr_fallbacks;      /* number of Cholesky pivots that had to be repaired since dlr_set_initial  */
+    int32_t nonfinite;         /* 1 if a non-finite value was seen in S                                    */
+} dlr_moments_t;
+
+typedef struct dlr_ctx dlr_ctx;
+
+/* Size in bytes of the single device workspace a context for cfg needs. Pure. */
+int dlr_workspace_bytes(const dlr_config* cfg, size_t* bytes);
+
+/* Create a context. d_workspace: DEVICE pointer, 256-byte aligned, >= dlr_workspace_bytes, owned by the
+ * caller (e.g. a torch.empty tensor) and kept alive until dlr_destroy. cuda_stream: a cudaStream_t (0 = the
+ * legacy default stream) on which ALL work of this context is issued. Builds wavenumber/twiddle tables. */
+int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cuda_stream, dlr_ctx** out);
+
+/* Copy in the initial factors (Algorithm 2 "Input"). X: N_x*r, S: r*r, V: N_v*r doubles in the
+ * layout above; on_device != 0: the three pointers are device pointers. Checks h^3 X^T X = I, h^3 V^T V = I
+ * to 1e-10 (DLR_ERR_NOT_ORTHONORMAL). S may be singular. The caller keeps its buffers. Synchronises. */
+int dlr_set_initial(dlr_ctx* ctx, const double* X, const double* S, const double* V, int on_device);
+
+/* One step of Algorithm 2 (order 1: Algorithm 1) of size tau: (X,S,V) <- (X3,S7,V1).
+ * Asynchronous on the context's stream; returns launch errors only. Numerical status is latched and
+ * read through dlr_moments. */
+int dlr_step(dlr_ctx* ctx, double tau);
+
+/* nsteps steps of size tau (same as calling dlr_step nsteps times). */
+int dlr_run(dlr_ctx* ctx, double tau, int nsteps);
+
+/* Diagnostics of the current state; optionally f at n_probe grid-index pairs:
+ * f_probe[p] = X[probe_ix[p],:] S V[probe_iv[p],:]^T (rows of F = X S V^T). probe_ix, probe_iv,
+ * f_probe are HOST arrays (may be NULL with n_probe = 0). Synchronises the stream. */
+int dlr_moments(dlr_ctx* ctx, dlr_moments_t* out, int n_probe, const int64_t* probe_ix,
+                const int64_t* probe_iv, double* f_probe);
+
+/* Copy out the current factors (checkpoint / tests). Factors are defined only up to the gauge
+ * X -> X Q1, V -> V Q2, S -> Q1^T S Q2. Any of X, S, V may be NULL. Synchronises. */
+int dlr_get_factors(dlr_ctx* ctx, double* X, double* S, double* V, int on_device);
+
+/* The electric field used last inside dlr_step (E^{1/2} of Algorithm 2 line 2; E^0 for order 1):
+ * 3*N_x doubles, component-major. For tests. */
+int dlr_get_field(dlr_ctx* ctx, double* E, int on_device);
+
+/* Per-phase device times (ms) of the LAST dlr_step executed with profiling on (dlr_set_profiling(ctx,1)
+ * makes dlr_step record CUDA events between phases and disables graph replay). names: the rows of the
+ * paper's Table 2. Returns the number of phases written (<= cap). */
+int dlr_set_profiling(dlr_ctx* ctx, int on);
+int dlr_get_phase_times(dlr_ctx* ctx, int cap, float* ms, const char** names);
+
+/* Number of kernel launches one dlr_step issues (for bench.py's gpu_launches). */
+int dlr_launches_per_step(dlr_ctx* ctx);
+
+/* Algorithmic bytes one dlr_step moves under the byte model of DESIGN.md section 6 (for the roofline). */
+double dlr_bytes_per_step(dlr_ctx* ctx);
+
+/* Kernel-level entry points for tests and micro-benchmarks (all pointers DEVICE, stream of ctx):
+ * batched 3D real-to-complex FFT of ncols columns on the x grid (which = 0) or v grid (which = 1) into the
+ * library's internal half-spectrum layout, and back (out = in up to rounding).  ncols must be the rank, 1 or 3. */
+int dlr_test_fft_roundtrip(dlr_ctx* ctx, int which, int ncols, const double* d_in, double* d_out,
+                           double* d_spec /* 2*ncols*(n/2+1)*n*n doubles */);
+
+void dlr_destroy(dlr_ctx* ctx);
+const char* dlr_strerror(int code);
+const char* dlr_last_cuda_error(dlr_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DLR_B200_H */

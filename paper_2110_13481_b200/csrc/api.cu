@@ -1,0 +1,811 @@
+// C ABI of include/dlr.h: context, workspace carving, and the orchestration of one step of Algorithm 2
+// / Algorithm 1 as a fixed sequence of kernels on one stream, replayed as a
+// CUDA graph.  No CPU fallback anywhere: every stage is a kernel launch.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/dlr.h"
+#include "rank_ops.h"
+#include "small.cuh"
+
+extern "C" {
+const RankOps* dlr_rank_ops_5();
+const RankOps* dlr_rank_ops_8();
+const RankOps* dlr_rank_ops_10();
+const RankOps* dlr_rank_ops_15();
+const RankOps* dlr_rank_ops_20();
+}
+
+const RankOps* dlr_rank_ops(int R) {
+    switch (R) {
+        case 5: return dlr_rank_ops_5();
+        case 8: return dlr_rank_ops_8();
+        case 10: return dlr_rank_ops_10();
+        case 15: return dlr_rank_ops_15();
+        case 20: return dlr_rank_ops_20();
+        default: return nullptr;
+    }
+}
+
+namespace {
+
+struct HostGrid {
+    GridDev g;
+    int T1;               // rows per CTA in dimension-1 passes (rank columns)
+    int T1s;              // same for the 1..3 column field passes
+    int T3, T3s;          // pencils per CTA in dimension-3 passes
+    int T2, NB2, nch2;    // dimension-2 pass tiling
+};
+
+struct FlowTab {
+    FlowTabPtrs p;
+};
+
+struct Phase {
+    const char* name;
+    cudaEvent_t ev;
+};
+
+}  // namespace
+
+struct dlr_ctx {
+    dlr_config cfg;
+    int R;
+    cudaStream_t st, cap_st;
+    const RankOps* ops;
+    HostGrid gx, gv;
+    // big buffers
+    double *X, *V, *S, *Sp;
+    double2 *Xh0, *Xh, *Vh, *W, *MB, *Eh;
+    double *KL, *Q1, *E;
+    double *partial, *partial2a, *partial2b;
+    // small buffers
+    double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *pvec, *zsum, *mx, *mv, *mres, *esum;
+    int* status;
+    long long *pix, *piv;
+    double* pf;
+    int probe_cap;
+    FlowTab ft;
+    double* small_end;
+    bool has_state, vh_valid, profiling;
+    int launches, count_launches;
+    cudaGraphExec_t graph;
+    double graph_tau;
+    cudaError_t last_err;
+    std::string last_err_msg;
+    std::vector<Phase> phases;
+    std::vector<float> phase_ms;
+    std::vector<const char*> phase_names;
+    size_t partial_cap;
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+int ilog2(int n) { int l = 0; while ((1 << l) < n) l++; return l; }
+int brev_host(int k, int bits) { int r = 0; for (int i = 0; i < bits; i++) if (k & (1 << i)) r |= 1 << (bits - 1 - i); return r; }
+
+// ---- tiling choices (shared-memory budget: <= ~110 KB so that two CTAs fit an SM when the problem allows) ----
+const size_t SMEM_TARGET = 110 * 1024, SMEM_MAX = 227 * 1024;
+
+int choose_T1(int n, int RMAX, bool needE, int nmat) {
+    const long long rows = (long long)n * n;
+    int best = 1;
+    for (int T = 1; T <= rows && T <= 64; T *= 2) {
+        const size_t sm = d1_smem_bytes(n, RMAX, T, needE, nmat);
+        if (sm > SMEM_TARGET && T > 1) break;
+        if (rows / T >= 296 || T <= 4) best = T;
+    }
+    while (best > 1 && d1_smem_bytes(n, RMAX, best, needE, nmat) > SMEM_MAX) best /= 2;
+    return best;
+}
+
+int choose_T3(int n, int RMAX, int nmat) {
+    int best = 1;
+    for (int T = 1; T <= 16; T *= 2) {
+        const size_t sm = d3_smem_bytes(n, RMAX, T, nmat);
+        if (sm <= SMEM_TARGET || (T <= 2 && sm <= SMEM_MAX)) best = T;
+    }
+    return best;
+}
+
+void choose_T2(int n, int nh, int& T2, int& NB, int& nch) {
+    int lines = (int)(SMEM_TARGET / ((size_t)n * 16));
+    if (lines > 255) lines = 255;
+    if (lines < 1) lines = 1;
+    nch = (nh + lines - 1) / lines;
+    T2 = (nh + nch - 1) / nch;
+    NB = lines / T2;
+    if (NB < 1) NB = 1;
+    if (NB > 16) NB = 16;
+}
+
+struct Carver {
+    char* base;
+    size_t off;
+    template <class Tp>
+    Tp* take(size_t count) {
+        off = align_up(off, 256);
+        Tp* p = base ? (Tp*)(base + off) : nullptr;
+        off += count * sizeof(Tp);
+        return p;
+    }
+};
+
+int check_cfg(const dlr_config* c) {
+    if (!c) return DLR_ERR_INVALID;
+    for (int d = 1; d < 3; d++)
+        if (c->n_x[d] != c->n_x[0] || c->n_v[d] != c->n_v[0]) return DLR_ERR_UNSUPPORTED;
+    const int nx = c->n_x[0], nv = c->n_v[0];
+    if (!is_pow2(nx) || !is_pow2(nv) || nx < 8 || nv < 8 || nx > 256 || nv > 256) return DLR_ERR_UNSUPPORTED;
+    if (!dlr_rank_ops(c->rank)) return DLR_ERR_UNSUPPORTED;
+    if (c->order != 1 && c->order != 2) return DLR_ERR_INVALID;
+    if (c->flags != 0) return DLR_ERR_INVALID;
+    for (int d = 0; d < 3; d++) {
+        if (!(c->x_hi[d] > c->x_lo[d]) || !(c->v_hi[d] > c->v_lo[d])) return DLR_ERR_INVALID;
+        if (c->x_lo[d] != c->x_lo[0] || c->x_hi[d] != c->x_hi[0] || c->v_lo[d] != c->v_lo[0] || c->v_hi[d] != c->v_hi[0])
+            return DLR_ERR_UNSUPPORTED;     // cubic boxes only (all configs of BASELINE.json)
+    }
+    return DLR_OK;
+}
+
+size_t grid_table_doubles(int n) { return (size_t)(2 * (n / 2 + 1) + 2 * n + n) + 8; }
+
+// carve the workspace; with base == nullptr only measures
+size_t carve(dlr_ctx* c, char* base) {
+    const int R = c->R;
+    const long long Nx = c->gx.g.N, Nv = c->gv.g.N, NCx = c->gx.g.NC, NCv = c->gv.g.NC;
+    const long long Nmax = Nx > Nv ? Nx : Nv, NCmax = NCx > NCv ? NCx : NCv;
+    Carver cv{base, 0};
+    c->X = cv.take<double>((size_t)Nx * R);
+    c->V = cv.take<double>((size_t)Nv * R);
+    c->KL = cv.take<double>((size_t)Nmax * R);
+    c->Q1 = cv.take<double>((size_t)Nmax * R);
+    c->Xh0 = cv.take<double2>((size_t)NCx * R);
+    c->Xh = cv.take<double2>((size_t)NCx * R);
+    c->Vh = cv.take<double2>((size_t)NCv * R);
+    c->W = cv.take<double2>((size_t)NCmax * R);
+    c->MB = cv.take<double2>((size_t)NCmax * R);
+    c->E = cv.take<double>((size_t)3 * Nx);
+    c->Eh = cv.take<double2>((size_t)3 * NCx);
+    // per-CTA partial sums: the largest producer is a dimension-1 pass with the weighted Gram
+    const int nvmax = 3 * R * (R + 1) / 2 + R;
+    size_t blocks = 0;
+    for (const HostGrid* hg : {&c->gx, &c->gv}) {
+        size_t b1 = (size_t)hg->g.n * hg->g.n / hg->T1;
+        size_t b3 = ((size_t)hg->g.nh * hg->g.n + hg->T3 - 1) / hg->T3;
+        blocks = std::max(blocks, std::max(b1, b3));
+    }
+    c->partial_cap = blocks * nvmax;
+    c->partial = cv.take<double>(c->partial_cap);
+    c->partial2a = cv.take<double>((size_t)DLR_G1 * nvmax);
+    c->partial2b = cv.take<double>((size_t)DLR_G1 * nvmax);
+    const int RR = R * R;
+    c->S = cv.take<double>(RR); c->Sp = cv.take<double>(RR);
+    c->C1 = cv.take<double>(3 * RR); c->C2 = cv.take<double>(3 * RR);
+    c->D1 = cv.take<double>(3 * RR); c->D2 = cv.take<double>(3 * RR);
+    c->rho_t = cv.take<double>(R);
+    c->TC = cv.take<double>(3 * RR); c->lamC = cv.take<double>(3 * R);
+    c->TD = cv.take<double>(3 * RR); c->lamD = cv.take<double>(3 * R);
+    c->apply = cv.take<double>(RR); c->Rtot = cv.take<double>(RR);
+    c->pvec = cv.take<double>(R); c->zsum = cv.take<double>(R);
+    c->mx = cv.take<double>(5 * R); c->mv = cv.take<double>(5 * R); c->mres = cv.take<double>(8); c->esum = cv.take<double>(2);
+    c->status = cv.take<int>(4);
+    c->probe_cap = 4096;
+    c->pix = cv.take<long long>(c->probe_cap); c->piv = cv.take<long long>(c->probe_cap); c->pf = cv.take<double>(c->probe_cap);
+    const int nmax = std::max(c->gx.g.n, c->gv.g.n), nhmax = nmax / 2 + 1;
+    c->ft.p.mats = cv.take<double>(8 * RR);
+    c->ft.p.nl = cv.take<double>(3 * RR);
+    c->ft.p.ph1 = cv.take<double2>((size_t)nhmax * R);
+    c->ft.p.ph2 = cv.take<double2>((size_t)nmax * R);
+    c->ft.p.ez = cv.take<double2>((size_t)nmax * R);
+    c->ft.p.f1 = cv.take<double2>((size_t)nmax * R);
+    c->ft.p.f2a = cv.take<double2>((size_t)nmax * R);
+    c->ft.p.f2b = cv.take<double2>((size_t)nmax * R);
+    // grid tables
+    for (HostGrid* hg : {&c->gx, &c->gv}) {
+        const int n = hg->g.n, nh = hg->g.nh;
+        double* t = cv.take<double>(grid_table_doubles(n));
+        hg->g.kt1 = t; hg->g.ksq1 = t ? t + nh : nullptr;
+        hg->g.kt2p = t ? t + 2 * nh : nullptr; hg->g.ksq2p = t ? t + 2 * nh + n : nullptr;
+        double2* tw = cv.take<double2>(n / 2);
+        hg->g.tw = tw;
+    }
+    return align_up(cv.off, 256);
+}
+
+void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
+    hg.g.n = n; hg.g.nh = n / 2 + 1; hg.g.log2n = ilog2(n);
+    hg.g.N = (long long)n * n * n; hg.g.NC = (long long)hg.g.nh * n * n;
+    hg.g.lo = lo; hg.g.h = (hi - lo) / n; hg.g.h3 = hg.g.h * hg.g.h * hg.g.h;
+    hg.T1 = choose_T1(n, R, true, 3 * R * R);
+    hg.T1s = choose_T1(n, 3, false, 4);
+    hg.T3 = choose_T3(n, R, 4 * R * R);
+    hg.T3s = choose_T3(n, 3, 0);
+    choose_T2(n, hg.g.nh, hg.T2, hg.NB2, hg.nch2);
+}
+
+cudaError_t upload_tables(dlr_ctx* c, HostGrid& hg, double lo, double hi) {
+    const int n = hg.g.n, nh = hg.g.nh, lg = hg.g.log2n;
+    const double L = hi - lo, PI = 3.14159265358979323846264338327950288;
+    std::vector<double> t(grid_table_doubles(n), 0.0);
+    for (int k = 0; k < nh; k++) {
+        const double kk = 2.0 * PI * k / L;
+        t[k] = (k == n / 2) ? 0.0 : kk;           // odd-derivative wavenumber, zero at Nyquist (R4)
+        t[nh + k] = kk * kk;                      // true k^2
+    }
+    for (int e = 0; e < n; e++) {
+        const int f = brev_host(e, lg);
+        const int m = f < n / 2 ? f : f - n;
+        const double kk = 2.0 * PI * m / L;
+        t[2 * nh + e] = (f == n / 2) ? 0.0 : kk;
+        t[2 * nh + n + e] = kk * kk;
+    }
+    cudaError_t e = cudaMemcpyAsync((void*)hg.g.kt1, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, c->st);
+    if (e != cudaSuccess) return e;
+    std::vector<double2> tw(n / 2);
+    for (int k = 0; k < n / 2; k++) {
+        const long double a = -2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)n;
+        tw[k] = make_double2((double)cosl(a), (double)sinl(a));
+    }
+    e = cudaMemcpyAsync((void*)hg.g.tw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice, c->st);
+    if (e != cudaSuccess) return e;
+    return cudaStreamSynchronize(c->st);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// launch helpers.  Every launch goes through CK so that the first failure is latched and counted.
+#define CK(expr)                                                      \
+    do {                                                              \
+        cudaError_t _e = (expr);                                      \
+        if (_e != cudaSuccess && c->last_err == cudaSuccess) {        \
+            c->last_err = _e;                                         \
+            c->last_err_msg = std::string(#expr) + ": " + cudaGetErrorString(_e); \
+        }                                                             \
+        c->count_launches++;                                          \
+    } while (0)
+
+void phase_mark(dlr_ctx* c, const char* name) {
+    if (!c->profiling) return;
+    Phase p;
+    p.name = name;
+    cudaEventCreate(&p.ev);
+    cudaEventRecord(p.ev, c->st);
+    c->phases.push_back(p);
+}
+
+void run_d2(dlr_ctx* c, const HostGrid& hg, double2* data, int ncols, bool inv) {
+    D2Args a;
+    a.g = hg.g; a.data = data; a.ncols = ncols; a.T2 = hg.T2; a.NB = hg.NB2; a.nchunks = hg.nch2;
+    if (inv) CK(launch_d2<true>(a, c->st)); else CK(launch_d2<false>(a, c->st));
+}
+
+D1Args d1args(const HostGrid& hg) {
+    D1Args a;
+    memset(&a, 0, sizeof(a));
+    a.g = hg.g; a.T = hg.T1; a.scale = 2.0 / (double)hg.g.N;
+    return a;
+}
+
+D3Args d3args(dlr_ctx* c, const HostGrid& hg) {
+    D3Args a;
+    memset(&a, 0, sizeof(a));
+    a.g = hg.g; a.T = hg.T3; a.e_scale = c->cfg.e_scale;
+    a.mats = c->ft.p.mats; a.ph1 = c->ft.p.ph1; a.ph2 = c->ft.p.ph2; a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1;
+    a.mbuf = c->MB;
+    return a;
+}
+
+void reduce_partials(dlr_ctx* c, int nblocks, int nvals, double* out2) {
+    k_reduce_partials<<<DLR_G1, 256, 0, c->st>>>(c->partial, nblocks, nvals, out2);
+    CK(cudaGetLastError());
+}
+
+int d1_blocks(const HostGrid& hg) { return (int)((long long)hg.g.n * hg.g.n / hg.T1); }
+int d3_blocks(const HostGrid& hg) { return (int)(((long long)hg.g.nh * hg.g.n + hg.T3 - 1) / hg.T3); }
+
+// Factor transform: A (real, N x r) -> Ah (half spectrum), accumulating the coefficient sums on the way:
+// kind = 0: none;  1: C coefficients (weights v_i, + rho_tilde);  2: D coefficients (weights E_i).
+void factor_fft(dlr_ctx* c, const HostGrid& hg, const double* A, double2* Ah, int kind, double* M1, double* M2,
+                double* colsum) {
+    const int R = c->R;
+    D1Args a = d1args(hg);
+    a.in_real = A; a.out_cplx = Ah; a.E = c->E; a.partial = c->partial;
+    CK(c->ops->d1[kind == 0 ? V1_FFT_PLAIN : kind == 1 ? V1_FFT_GRAMV : V1_FFT_GRAME](a, c->st));
+    if (kind) reduce_partials(c, d1_blocks(hg), d1_gram_nvals(R, kind == 1 ? D1_GRAM_V : D1_GRAM_E), c->partial2a);
+    run_d2(c, hg, Ah, R, false);
+    D3Args b = d3args(c, hg);
+    b.in = Ah; b.out = Ah; b.partial = c->partial;
+    CK(c->ops->d3[kind ? V3_FWD_PGRAM : V3_FWD](b, c->st));
+    if (kind) {
+        reduce_partials(c, d3_blocks(hg), 3 * R * (R - 1) / 2, c->partial2b);
+        k_finalize_coeff<<<1, 256, 0, c->st>>>(c->partial2a, c->partial2b, R, kind == 1, hg.g.h3, 1.0 / (double)hg.g.N,
+                                               M1, M2, colsum);
+        CK(cudaGetLastError());
+    }
+}
+
+void eig3(dlr_ctx* c, const double* M1, double* T, double* lam) {
+    k_eig3<<<1, 96, 0, c->st>>>(M1, c->R, T, lam);
+    CK(cudaGetLastError());
+}
+
+void sflow(dlr_ctx* c, double* S, double t) {
+    k_sflow<<<1, 256, 0, c->st>>>(S, c->R, t, c->C1, c->C2, c->D1, c->D2);
+    CK(cudaGetLastError());
+}
+
+// Electric field from rho = A * pvec (pvec already holds the minus sign and weights): eqs. (12)/(13) + Poisson
+// (PAPER.md:180-190):  r2c -> FFT2 -> FFT3, E_hat = -i kt phi_hat, back -> E (3 x N_x real).
+void field(dlr_ctx* c, const double* A) {
+    const HostGrid& hg = c->gx;
+    D1Args a = d1args(hg);
+    a.in_real = A; a.out_cplx = c->Eh; a.mat = c->pvec;
+    CK(c->ops->d1[V1_RHO](a, c->st));
+    run_d2(c, hg, c->Eh, 1, false);
+    D3Args b = d3args(c, hg);
+    b.in = c->Eh; b.out = c->Eh; b.T = hg.T3s;
+    CK((launch_d3<1, 3, D3_POISSON, false>(b, c->st)));
+    run_d2(c, hg, c->Eh, 3, true);
+    D1Args e = d1args(hg);
+    e.T = hg.T1s; e.in_cplx = c->Eh; e.out_real = c->E;
+    CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
+}
+
+// shifted CholeskyQR3 of KL (N x r) -> orthonormal basis (h^3 B^T B = I) into `basis`, coupling matrix into Sout
+// (transS: S = R^T for the L step, Fig. 1 line 40 transpose_inplace).
+// The Gram sums of KL must already be in c->partial (written by the pass that produced KL).
+void qr(dlr_ctx* c, const HostGrid& hg, double* basis, double* Sout, int transS) {
+    const int R = c->R, P = R * (R + 1) / 2;
+    const double shift = 64.0 * R * 2.220446049250313e-16;
+    const double osc = 1.0 / sqrt(hg.g.h3), ssc = sqrt(hg.g.h3);
+    double* src[3] = {c->KL, c->Q1, c->KL};
+    double* dst[3] = {c->Q1, c->KL, basis};
+    for (int stage = 0; stage < 3; stage++) {
+        reduce_partials(c, d1_blocks(hg), P, c->partial2a);
+        k_chol_stage<<<1, 32, 0, c->st>>>(c->partial2a, R, stage, stage == 2, shift, osc, ssc, transS, c->apply, c->Rtot,
+                                          Sout, c->status);
+        CK(cudaGetLastError());
+        D1Args a = d1args(hg);
+        a.in_real = src[stage]; a.out_real = dst[stage]; a.mat = c->apply; a.partial = c->partial;
+        CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
+    }
+}
+
+void flow_tables(dlr_ctx* c, const HostGrid& hg, const double* T, const double* lam, const double* Sin, int transS,
+                 double sgn, double tsub, double t3, const double* M2c, double nlsign) {
+    k_flow_tables<<<1, 256, 0, c->st>>>(T, lam, Sin, transS, c->R, hg.g, sgn, tsub, t3, M2c, nlsign, c->ft.p);
+    CK(cudaGetLastError());
+}
+
+// K- or L-flow of section 4 starting from the spectrum `spec` of the basis (the product with the
+// coupling matrix is folded into the first mode-mixing matrix).  order 1: Lie + exponential Euler; order 2: Strang +
+// ETD2RK.  Result: real factor in c->KL with its Gram sums in c->partial, or (zero_only) only the column sums of
+// the result (without the h^3 weight) in c->zsum.
+void flow(dlr_ctx* c, const HostGrid& hg, const double2* spec, bool is_L, int order, bool zero_only) {
+    const RankOps* ops = c->ops;
+    const int vmid = is_L ? V1_MID_V : V1_MID_E;
+    D3Args s = d3args(c, hg);
+    s.in = spec; s.out = c->W;
+    CK(ops->d3[V3_START](s, c->st));
+    run_d2(c, hg, c->W, c->R, true);
+    D1Args m = d1args(hg);
+    m.in_cplx = c->W; m.out_cplx = c->W; m.mat = c->ft.p.nl; m.E = c->E;
+    CK(ops->d1[vmid](m, c->st));
+    run_d2(c, hg, c->W, c->R, false);
+    D3Args e = d3args(c, hg);
+    e.in = c->W; e.out = c->W;
+    if (order == 1) {
+        if (zero_only) { e.zero_out = c->zsum; e.skip_store = 1; }
+        CK(ops->d3[V3_EULER_END](e, c->st));
+        if (zero_only) return;
+    } else {
+        e.f2 = c->ft.p.f2a;
+        CK(ops->d3[V3_MID](e, c->st));
+        run_d2(c, hg, c->W, c->R, true);
+        CK(ops->d1[vmid](m, c->st));
+        run_d2(c, hg, c->W, c->R, false);
+        e.f2 = c->ft.p.f2b;
+        CK(ops->d3[V3_END2](e, c->st));
+    }
+    run_d2(c, hg, c->W, c->R, true);
+    D1Args o = d1args(hg);
+    o.in_cplx = c->W; o.out_real = c->KL; o.partial = c->partial;
+    CK(ops->d1[V1_INV_GRAM](o, c->st));
+}
+
+void rho_vec(dlr_ctx* c, const double* S, const double* vec, int use_S, double scale) {
+    k_rho_vec<<<1, 32, 0, c->st>>>(S, vec, c->R, use_S, scale, c->pvec);
+    CK(cudaGetLastError());
+}
+
+// one step, issued on c->st (directly or under stream capture)
+void issue_step(dlr_ctx* c, double tau) {
+    const int order = c->cfg.order;
+    const double tp = order == 2 ? 0.5 * tau : tau;     // step size of the Algorithm-1 part
+    const HostGrid &gx = c->gx, &gv = c->gv;
+    double* Sp = order == 2 ? c->Sp : c->S;             // the predictor of Algorithm 2 works on a scratch S
+    phase_mark(c, "start");
+    // ---- Algorithm 1, line 1: C coefficients from V0 (kept from the previous step's line 10 when valid)
+    if (!c->vh_valid) {
+        factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->C2, c->rho_t);
+        eig3(c, c->C1, c->TC, c->lamC);
+    }
+    phase_mark(c, "C coefficients (V0)");
+    // ---- line 2: K0 = X0 S0, kept as the spectrum of X0 (the product with S0 is folded into the flow)
+    factor_fft(c, gx, c->X, c->Xh0, 0, nullptr, nullptr, nullptr);
+    // ---- line 3: E0 from K0 and V0, eq. (12): rho = -X0 (S0 rho_tilde)
+    rho_vec(c, c->S, c->rho_t, 1, -1.0);
+    field(c, c->X);
+    phase_mark(c, "electric field E0");
+    // ---- line 4: K step (Lie, exponential Euler) of length tp with E0;  line 5: QR -> X1, S1
+    flow_tables(c, gx, c->TC, c->lamC, c->S, 0, -1.0, tp, tp, c->C2, 1.0);
+    flow(c, gx, c->Xh0, false, 1, false);
+    phase_mark(c, "K step (predictor)");
+    qr(c, gx, c->X, Sp, 0);
+    phase_mark(c, "QR K (predictor)");
+    // ---- line 6: D coefficients from X1 and E0
+    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, c->D2, nullptr);
+    eig3(c, c->D1, c->TD, c->lamD);
+    phase_mark(c, "D coefficients (predictor)");
+    // ---- line 7: S step
+    sflow(c, Sp, tp);
+    phase_mark(c, "S step (predictor)");
+    // ---- lines 8-9: L0 = V0 S2^T, L step with E0
+    flow_tables(c, gv, c->TD, c->lamD, Sp, 1, +1.0, tp, tp, c->D2, -1.0);
+    if (order == 1) {
+        flow(c, gv, c->Vh, true, 1, false);
+        phase_mark(c, "L step");
+        qr(c, gv, c->V, c->S, 1);                 // line 10: V1, S3 = R^T
+        phase_mark(c, "QR L");
+        c->vh_valid = false;
+        return;
+    }
+    flow(c, gv, c->Vh, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
+    phase_mark(c, "L step (predictor)");
+    // ---- Algorithm 2, line 2: E^{1/2} from X1 and L1, eq. (13)
+    rho_vec(c, c->S, c->zsum, 0, -gv.g.h3);
+    field(c, c->X);
+    phase_mark(c, "electric field E1/2");
+    // ---- line 3: K step (Strang, ETD2RK) of length tau/2 from K0 = X0 S0 with E^{1/2};  line 4: QR -> X2, S3
+    flow_tables(c, gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0);
+    flow(c, gx, c->Xh0, false, 2, false);
+    phase_mark(c, "first K step");
+    qr(c, gx, c->X, c->S, 0);
+    phase_mark(c, "QR K (first)");
+    // ---- line 5: D coefficients from X2 and E^{1/2};  line 6: S step
+    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, c->D2, nullptr);
+    eig3(c, c->D1, c->TD, c->lamD);
+    phase_mark(c, "D coefficients");
+    sflow(c, c->S, 0.5 * tau);
+    phase_mark(c, "first S step");
+    // ---- lines 7-9: L = V0 S4^T, L step (Strang) of length tau, QR -> V1, S5 = R^T
+    flow_tables(c, gv, c->TD, c->lamD, c->S, 1, +1.0, 0.5 * tau, tau, c->D2, -1.0);
+    flow(c, gv, c->Vh, true, 2, false);
+    phase_mark(c, "L step");
+    qr(c, gv, c->V, c->S, 1);
+    phase_mark(c, "QR L");
+    // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step
+    factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->C2, c->rho_t);
+    eig3(c, c->C1, c->TC, c->lamC);
+    phase_mark(c, "C coefficients");
+    sflow(c, c->S, 0.5 * tau);
+    phase_mark(c, "second S step");
+    // ---- lines 12-14: K3 = X2 S6 (spectrum of X2 is in Xh), K step (Strang) of length tau/2, QR -> X3, S7
+    flow_tables(c, gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0);
+    flow(c, gx, c->Xh, false, 2, false);
+    phase_mark(c, "second K step");
+    qr(c, gx, c->X, c->S, 0);
+    phase_mark(c, "QR K (second)");
+    c->vh_valid = true;
+}
+
+int fail(dlr_ctx* c, cudaError_t e, const char* what) {
+    if (c && c->last_err == cudaSuccess) {
+        c->last_err = e;
+        c->last_err_msg = std::string(what) + ": " + cudaGetErrorString(e);
+    }
+    return DLR_ERR_CUDA;
+}
+
+}  // namespace
+
+// =========================================================================================================
+extern "C" {
+
+const char* dlr_strerror(int code) {
+    switch (code) {
+        case DLR_OK: return "ok";
+        case DLR_ERR_INVALID: return "invalid argument";
+        case DLR_ERR_UNSUPPORTED: return "unsupported grid size or rank";
+        case DLR_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case DLR_ERR_CUDA: return "CUDA error";
+        case DLR_ERR_NOT_ORTHONORMAL: return "initial factors are not orthonormal";
+        case DLR_ERR_NO_STATE: return "no state set";
+        default: return "unknown error";
+    }
+}
+
+const char* dlr_last_cuda_error(dlr_ctx* c) { return c ? c->last_err_msg.c_str() : ""; }
+
+static void init_grids(dlr_ctx* c) {
+    setup_grid(c->gx, c->cfg.n_x[0], c->cfg.x_lo[0], c->cfg.x_hi[0], c->R);
+    setup_grid(c->gv, c->cfg.n_v[0], c->cfg.v_lo[0], c->cfg.v_hi[0], c->R);
+}
+
+int dlr_workspace_bytes(const dlr_config* cfg, size_t* bytes) {
+    if (!bytes) return DLR_ERR_INVALID;
+    int rc = check_cfg(cfg);
+    if (rc != DLR_OK) return rc;
+    dlr_ctx tmp{};
+    tmp.cfg = *cfg; tmp.R = cfg->rank;
+    init_grids(&tmp);
+    *bytes = carve(&tmp, nullptr);
+    return DLR_OK;
+}
+
+int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cuda_stream, dlr_ctx** out) {
+    if (!out || !d_workspace) return DLR_ERR_INVALID;
+    int rc = check_cfg(cfg);
+    if (rc != DLR_OK) return rc;
+    if (((uintptr_t)d_workspace & 255) != 0) return DLR_ERR_WORKSPACE;
+    dlr_ctx* c = new dlr_ctx{};
+    c->cfg = *cfg; c->R = cfg->rank; c->st = (cudaStream_t)cuda_stream; c->ops = dlr_rank_ops(cfg->rank);
+    c->last_err = cudaSuccess;
+    init_grids(c);
+    const size_t need = carve(c, (char*)d_workspace);
+    if (need > bytes) { delete c; return DLR_ERR_WORKSPACE; }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) { delete c; return DLR_ERR_CUDA; }
+    e = cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
+    e = upload_tables(c, c->gx, cfg->x_lo[0], cfg->x_hi[0]);
+    if (e == cudaSuccess) e = upload_tables(c, c->gv, cfg->v_lo[0], cfg->v_hi[0]);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->status, 0, 4 * sizeof(int), c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
+    *out = c;
+    return DLR_OK;
+}
+
+void dlr_destroy(dlr_ctx* c) {
+    if (!c) return;
+    if (c->graph) cudaGraphExecDestroy(c->graph);
+    if (c->cap_st) cudaStreamDestroy(c->cap_st);
+    for (auto& p : c->phases) cudaEventDestroy(p.ev);
+    delete c;
+}
+
+static int gram_check(dlr_ctx* c, const HostGrid& hg, const double* A) {
+    const int R = c->R, P = R * (R + 1) / 2;
+    D1Args a = d1args(hg);
+    a.in_real = A; a.partial = c->partial;
+    CK(c->ops->d1[V1_GRAM_ONLY](a, c->st));
+    reduce_partials(c, d1_blocks(hg), P, c->partial2a);
+    std::vector<double> h((size_t)DLR_G1 * P);
+    cudaError_t e = cudaMemcpyAsync(h.data(), c->partial2a, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) return fail(c, e, "gram_check");
+    if (c->last_err != cudaSuccess) return DLR_ERR_CUDA;
+    int idx = 0;
+    for (int a1 = 0; a1 < R; a1++)
+        for (int b = a1; b < R; b++, idx++) {
+            double s = 0.0;
+            for (int g = 0; g < DLR_G1; g++) s += h[(size_t)g * P + idx];
+            if (!(fabs(s * hg.g.h3 - (a1 == b ? 1.0 : 0.0)) <= 1e-10)) return DLR_ERR_NOT_ORTHONORMAL;
+        }
+    return DLR_OK;
+}
+
+int dlr_set_initial(dlr_ctx* c, const double* X, const double* S, const double* V, int on_device) {
+    if (!c || !X || !S || !V) return DLR_ERR_INVALID;
+    const cudaMemcpyKind k = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    const int R = c->R;
+    cudaError_t e = cudaMemcpyAsync(c->X, X, (size_t)c->gx.g.N * R * sizeof(double), k, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->V, V, (size_t)c->gv.g.N * R * sizeof(double), k, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->S, S, (size_t)R * R * sizeof(double), k, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->status, 0, 4 * sizeof(int), c->st);
+    if (e != cudaSuccess) return fail(c, e, "dlr_set_initial copy");
+    c->vh_valid = false;
+    c->has_state = false;
+    int rc = gram_check(c, c->gx, c->X);
+    if (rc == DLR_OK) rc = gram_check(c, c->gv, c->V);
+    if (rc != DLR_OK) return rc;
+    c->has_state = true;
+    return DLR_OK;
+}
+
+int dlr_step(dlr_ctx* c, double tau) {
+    if (!c) return DLR_ERR_INVALID;
+    if (!c->has_state) return DLR_ERR_NO_STATE;
+    if (c->last_err != cudaSuccess) return DLR_ERR_CUDA;
+    if (c->profiling || !c->vh_valid) {
+        // first step after set_initial (it also computes the C coefficients of V0) or profiling: direct launches
+        for (auto& p : c->phases) cudaEventDestroy(p.ev);
+        c->phases.clear();
+        c->count_launches = 0;
+        issue_step(c, tau);
+        return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;
+    }
+    if (!c->graph || c->graph_tau != tau) {
+        if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+        // warm every kernel's attributes outside capture is unnecessary: they were all launched by the first step
+        cudaGraph_t g;
+        // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
+        // the instantiated graph is then launched on the caller's stream
+        cudaStream_t user = c->st;
+        cudaError_t e = cudaStreamBeginCapture(c->cap_st, cudaStreamCaptureModeThreadLocal);
+        if (e != cudaSuccess) return fail(c, e, "begin capture");
+        c->count_launches = 0;
+        c->st = c->cap_st;
+        issue_step(c, tau);
+        c->st = user;
+        e = cudaStreamEndCapture(c->cap_st, &g);
+        if (e != cudaSuccess) return fail(c, e, "end capture");
+        if (c->last_err != cudaSuccess) { cudaGraphDestroy(g); return DLR_ERR_CUDA; }
+        c->launches = c->count_launches;
+        e = cudaGraphInstantiate(&c->graph, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) return fail(c, e, "graph instantiate");
+        c->graph_tau = tau;
+    }
+    cudaError_t e = cudaGraphLaunch(c->graph, c->st);
+    if (e != cudaSuccess) return fail(c, e, "graph launch");
+    return DLR_OK;
+}
+
+int dlr_run(dlr_ctx* c, double tau, int nsteps) {
+    for (int i = 0; i < nsteps; i++) {
+        int rc = dlr_step(c, tau);
+        if (rc != DLR_OK) return rc;
+    }
+    return DLR_OK;
+}
+
+int dlr_launches_per_step(dlr_ctx* c) { return c ? (c->launches ? c->launches : c->count_launches) : 0; }
+
+double dlr_bytes_per_step(dlr_ctx* c) {
+    // byte model of DESIGN.md section 6 (fused design): 110 * B with B = 8 N r per factor;
+    // for N_x != N_v the K-side and L-side shares are weighted 64:46.
+    if (!c) return 0.0;
+    const double Bx = 8.0 * (double)c->gx.g.N * c->R, Bv = 8.0 * (double)c->gv.g.N * c->R;
+    return c->cfg.order == 2 ? 64.0 * Bx + 46.0 * Bv : 24.0 * Bx + 24.0 * Bv;
+}
+
+int dlr_set_profiling(dlr_ctx* c, int on) {
+    if (!c) return DLR_ERR_INVALID;
+    c->profiling = on != 0;
+    return DLR_OK;
+}
+
+int dlr_get_phase_times(dlr_ctx* c, int cap, float* ms, const char** names) {
+    if (!c) return 0;
+    cudaStreamSynchronize(c->st);
+    int n = 0;
+    for (size_t i = 1; i < c->phases.size() && n < cap; i++, n++) {
+        float t = 0.f;
+        cudaEventElapsedTime(&t, c->phases[i - 1].ev, c->phases[i].ev);
+        if (ms) ms[n] = t;
+        if (names) names[n] = c->phases[i].name;
+    }
+    return n;
+}
+
+int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* probe_ix, const int64_t* probe_iv,
+                double* f_probe) {
+    if (!c || !out) return DLR_ERR_INVALID;
+    if (!c->has_state) return DLR_ERR_NO_STATE;
+    if (n_probe < 0 || n_probe > c->probe_cap || (n_probe > 0 && (!probe_ix || !probe_iv || !f_probe))) return DLR_ERR_INVALID;
+    const int R = c->R;
+    k_colmoments<<<R, 1024, 0, c->st>>>(c->X, c->gx.g, c->mx);
+    CK(cudaGetLastError());
+    k_colmoments<<<R, 1024, 0, c->st>>>(c->V, c->gv.g, c->mv);
+    CK(cudaGetLastError());
+    k_moments_final<<<1, 32, 0, c->st>>>(c->mx, c->mv, c->S, R, c->gx.g.h3, c->gv.g.h3, c->mres);
+    CK(cudaGetLastError());
+    // electric energy: E from eq. (12) on the current factors.  rho_tilde = h_v^3 V^T 1 = h_v^3 * mv[:,0]
+    // (uses the scratch field buffers; the step does not depend on them across steps)
+    k_rho_vec<<<1, 32, 0, c->st>>>(c->S, c->mv, R, 2, -c->gv.g.h3, c->pvec);
+    CK(cudaGetLastError());
+    field(c, c->X);
+    k_sumsq<<<1, 1024, 0, c->st>>>(c->E, 3 * c->gx.g.N, c->esum);
+    CK(cudaGetLastError());
+    if (n_probe > 0) {
+        cudaError_t e = cudaMemcpyAsync(c->pix, probe_ix, n_probe * sizeof(int64_t), cudaMemcpyHostToDevice, c->st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(c->piv, probe_iv, n_probe * sizeof(int64_t), cudaMemcpyHostToDevice, c->st);
+        if (e != cudaSuccess) return fail(c, e, "probe upload");
+        k_probes<<<(n_probe + 127) / 128, 128, 0, c->st>>>(c->X, c->S, c->V, c->gx.g.N, c->gv.g.N, R, n_probe, c->pix, c->piv, c->pf);
+        CK(cudaGetLastError());
+    }
+    double res[8], es[2];
+    int st[4];
+    cudaError_t e = cudaMemcpyAsync(res, c->mres, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(es, c->esum, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st, c->status, 4 * sizeof(int), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess && n_probe > 0) e = cudaMemcpyAsync(f_probe, c->pf, n_probe * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) return fail(c, e, "dlr_moments");
+    if (c->last_err != cudaSuccess) return DLR_ERR_CUDA;
+    out->mass = res[0];
+    out->momentum[0] = res[1]; out->momentum[1] = res[2]; out->momentum[2] = res[3];
+    out->kinetic_energy = res[4];
+    out->s_fro = res[5];
+    out->nonfinite = res[6] != 0.0;
+    out->electric_energy = 0.5 * c->gx.g.h3 * es[0];
+    out->qr_fallbacks = st[0];
+    return DLR_OK;
+}
+
+int dlr_get_factors(dlr_ctx* c, double* X, double* S, double* V, int on_device) {
+    if (!c) return DLR_ERR_INVALID;
+    if (!c->has_state) return DLR_ERR_NO_STATE;
+    const cudaMemcpyKind k = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    const int R = c->R;
+    cudaError_t e = cudaSuccess;
+    if (X) e = cudaMemcpyAsync(X, c->X, (size_t)c->gx.g.N * R * sizeof(double), k, c->st);
+    if (e == cudaSuccess && V) e = cudaMemcpyAsync(V, c->V, (size_t)c->gv.g.N * R * sizeof(double), k, c->st);
+    if (e == cudaSuccess && S) e = cudaMemcpyAsync(S, c->S, (size_t)R * R * sizeof(double), k, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) return fail(c, e, "dlr_get_factors");
+    return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;
+}
+
+int dlr_get_field(dlr_ctx* c, double* E, int on_device) {
+    if (!c || !E) return DLR_ERR_INVALID;
+    cudaError_t e = cudaMemcpyAsync(E, c->E, (size_t)3 * c->gx.g.N * sizeof(double),
+                                    on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    return e == cudaSuccess ? DLR_OK : fail(c, e, "dlr_get_field");
+}
+
+int dlr_test_fft_roundtrip(dlr_ctx* c, int which, int ncols, const double* d_in, double* d_out, double* d_spec) {
+    if (!c || !d_in || !d_out || !d_spec) return DLR_ERR_INVALID;
+    const HostGrid& hg = which ? c->gv : c->gx;
+    double2* spec = (double2*)d_spec;
+    D1Args a = d1args(hg);
+    a.in_real = d_in; a.out_cplx = spec;
+    D3Args b = d3args(c, hg);
+    b.in = spec; b.out = spec;
+    D1Args e = d1args(hg);
+    e.in_cplx = spec; e.out_real = d_out;
+    if (ncols == c->R) {
+        CK(c->ops->d1[V1_FFT_PLAIN](a, c->st));
+        run_d2(c, hg, spec, ncols, false);
+        CK(c->ops->d3[V3_FWD](b, c->st));
+    } else if (ncols == 3) {
+        a.T = e.T = hg.T1s; b.T = hg.T3s;
+        CK((launch_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>(a, c->st)));
+        run_d2(c, hg, spec, ncols, false);
+        CK((launch_d3<3, 3, D3_FWD_STORE, false>(b, c->st)));
+    } else {
+        return DLR_ERR_UNSUPPORTED;
+    }
+    cudaError_t er = cudaStreamSynchronize(c->st);
+    if (er != cudaSuccess) return fail(c, er, "fft forward");
+    // the inverse consumes a copy so that d_spec keeps the forward transform for inspection
+    double2* tmp = c->W;
+    er = cudaMemcpyAsync(tmp, spec, (size_t)ncols * hg.g.NC * sizeof(double2), cudaMemcpyDeviceToDevice, c->st);
+    if (er != cudaSuccess) return fail(c, er, "fft copy");
+    b.in = tmp; b.out = tmp; e.in_cplx = tmp;
+    if (ncols == c->R) {
+        CK(c->ops->d3[V3_INV](b, c->st));
+        run_d2(c, hg, tmp, ncols, true);
+        CK(c->ops->d1[V1_INV](e, c->st));
+    } else {
+        CK((launch_d3<3, 3, D3_INV_ONLY, false>(b, c->st)));
+        run_d2(c, hg, tmp, ncols, true);
+        CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
+    }
+    er = cudaStreamSynchronize(c->st);
+    if (er != cudaSuccess) return fail(c, er, "fft inverse");
+    return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,138 @@
+// Shared device-side definitions of the DLR hot path (sm_100a, fp64).
+// Data layouts:
+//   real factor      A[c][i3][i2][i1]            column stride N = n^3, i1 fastest (the C ABI's column-major N x r)
+//   half spectrum    Ah[c][k3'][k2'][k1]         column stride NC = (n/2+1) n^2 complex; k1 = 0..n/2 in natural
+//                    order, k2', k3' are BIT-REVERSED positions (decimation-in-frequency forward transforms leave
+//                    them there; decimation-in-time inverses consume them; all wavenumber tables are built in
+//                    stored-position order, so no kernel ever reorders data).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define DLR_THREADS 256
+
+struct GridDev {
+    int n, nh, log2n;        // points per dimension, n/2+1, log2(n)
+    long long N, NC;         // n^3, nh*n*n
+    double lo, h, h3;        // left extreme, spacing, h^3
+    const double* kt1;       // [nh]  odd-derivative wavenumber by k1 (0 at Nyquist)            (reading R4)
+    const double* kt2p;      // [n]   same, by stored (bit-reversed) position in dims 2,3
+    const double* ksq1;      // [nh]  true k^2 by k1
+    const double* ksq2p;     // [n]   true k^2 by stored position
+    const double2* tw;       // [n/2] exp(-2 pi i k / n)
+};
+
+// ---------------------------------------------------------------- complex helpers
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ double2 cmulc(double2 a, double2 b) {   // a * conj(b)
+    return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -a.x * b.y));
+}
+__device__ __forceinline__ double2 cconj(double2 a) { return make_double2(a.x, -a.y); }
+
+// ---------------------------------------------------------------- shared-memory FFT over many lines
+// Lines live in shared memory as s[elem * LP + line] (line index fastest => consecutive threads touch
+// consecutive 16-byte words: conflict-free in every stage, twiddles are warp-uniform).
+// Forward = decimation in frequency, natural order in -> bit-reversed order out, kernel exp(-2 pi i jk/M).
+// Inverse = the exact transpose: bit-reversed in -> natural out, conjugate twiddles, unnormalised.
+// tw[] holds exp(-2 pi i k / TWN), k < TWN/2, with TWN = M * twmul.
+template <int G, bool INV>
+__device__ __forceinline__ void fft_group(double2* s, int LP, int nlines, int M, int lev0, const double2* tw,
+                                          int twmul) {
+    constexpr int R = 1 << G;
+    const int B = M >> lev0;          // block size at the first (coarsest) level of the group
+    const int st = B >> G;            // element stride between the R registers
+    const int items = (M >> G) * nlines;
+    for (int w = threadIdx.x; w < items; w += blockDim.x) {
+        const int line = w % nlines;
+        const int it = w / nlines;
+        const int j = it % st;
+        const int b = it / st;
+        double2* p = s + (size_t)(b * B + j) * LP + line;
+        double2 a[R];
+#pragma unroll
+        for (int q = 0; q < R; q++) a[q] = p[(size_t)q * st * LP];
+        if (!INV) {
+#pragma unroll
+            for (int lv = 0; lv < G; lv++) {
+                const int hq = R >> (lv + 1);
+                const int mul = twmul << (lev0 + lv);      // M/(2h) * twmul with 2h = B >> lv
+#pragma unroll
+                for (int q = 0; q < R; q++) {
+                    if ((q & hq) == 0) {
+                        const int pos = j + (q & (hq - 1)) * st;
+                        double2 u = a[q], v = a[q + hq];
+                        a[q] = cadd(u, v);
+                        a[q + hq] = cmul(csub(u, v), tw[pos * mul]);
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int lv = G - 1; lv >= 0; lv--) {
+                const int hq = R >> (lv + 1);
+                const int mul = twmul << (lev0 + lv);
+#pragma unroll
+                for (int q = 0; q < R; q++) {
+                    if ((q & hq) == 0) {
+                        const int pos = j + (q & (hq - 1)) * st;
+                        double2 u = a[q];
+                        double2 t = cmulc(a[q + hq], tw[pos * mul]);
+                        a[q] = cadd(u, t);
+                        a[q + hq] = csub(u, t);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < R; q++) p[(size_t)q * st * LP] = a[q];
+    }
+}
+
+// level grouping for log2(M) = 2..8 (each group = one pass over shared memory)
+__device__ __forceinline__ void fft_plan(int logM, int g[3], int& ng) {
+    switch (logM) {
+        case 1: g[0] = 1; ng = 1; break;
+        case 2: g[0] = 2; ng = 1; break;
+        case 3: g[0] = 3; ng = 1; break;
+        case 4: g[0] = 2; g[1] = 2; ng = 2; break;
+        case 5: g[0] = 3; g[1] = 2; ng = 2; break;
+        case 6: g[0] = 3; g[1] = 3; ng = 2; break;
+        case 7: g[0] = 3; g[1] = 2; g[2] = 2; ng = 3; break;
+        default: g[0] = 3; g[1] = 3; g[2] = 2; ng = 3; break;
+    }
+}
+
+template <bool INV>
+__device__ __forceinline__ void fft_lines(double2* s, int LP, int nlines, int logM, const double2* tw, int twmul) {
+    int g[3], ng;
+    fft_plan(logM, g, ng);
+    const int M = 1 << logM;
+    int lev[3];
+    lev[0] = 0;
+    lev[1] = g[0];
+    lev[2] = g[0] + g[1];
+    for (int ii = 0; ii < ng; ii++) {
+        const int i = INV ? ng - 1 - ii : ii;
+        switch (g[i]) {
+            case 1: fft_group<1, INV>(s, LP, nlines, M, lev[i], tw, twmul); break;
+            case 2: fft_group<2, INV>(s, LP, nlines, M, lev[i], tw, twmul); break;
+            default: fft_group<3, INV>(s, LP, nlines, M, lev[i], tw, twmul); break;
+        }
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ int brev(int k, int logM) { return (int)(__brev((unsigned)k) >> (32 - logM)); }
+
+// ---------------------------------------------------------------- warp-owned Gram accumulation
+// Each warp owns a contiguous range of the output entries; for every entry it sweeps all points of the
+// tile (lane-strided), reduces by shuffles and lane 0 writes the partial: no atomics, fixed order.
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}

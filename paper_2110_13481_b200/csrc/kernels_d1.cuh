@@ -1,0 +1,257 @@
+// Dimension-1 pass: everything that happens while a tile of grid rows (lines along i1) of ALL columns sits in
+// shared memory in real space:
+//   load (real rows, or half-spectrum rows + complex-to-real inverse transform along dim 1)
+//   -> point-wise operation across the columns (K = A*Mat; the non-diagonal terms of eqs. (9)/(11))
+//   -> weighted Gram accumulation (C1/D1 of PAPER.md:150,162; rho_tilde of eq. (12); Gram matrix for CholeskyQR)
+//   -> store (real rows and/or real-to-complex forward transform along dim 1 into the half spectrum).
+// A real row of n doubles is handled as n/2 complex numbers z[j] = a[2j] + i a[2j+1] (half-length complex FFT
+// + split/merge step), so the real data never needs a repacking pass.
+#pragma once
+#include "common.cuh"
+
+enum { D1_IN_REAL = 0, D1_IN_CPLX = 1 };
+enum { D1_OP_NONE = 0, D1_OP_MATVEC = 1, D1_OP_NONLIN_E = 2, D1_OP_NONLIN_V = 3 };
+enum { D1_GRAM_NONE = 0, D1_GRAM_PLAIN = 1, D1_GRAM_V = 2, D1_GRAM_E = 3 };
+enum { D1_OUT_NONE = 0, D1_OUT_REAL = 1, D1_OUT_CPLX = 2, D1_OUT_BOTH = 3 };
+
+struct D1Args {
+    GridDev g;
+    const double* in_real;     // RIN columns, stride N
+    const double2* in_cplx;    // RIN columns, stride NC
+    double* out_real;          // ROUT columns
+    double2* out_cplx;         // ROUT columns
+    const double* mat;         // MATVEC: [RIN][ROUT];  NONLIN: 3 x [R][R], out_c = sum_i w_i sum_c' M_i[c][c'] a_c'
+    const double* E;           // [3][N] weights for NONLIN_E / GRAM_E
+    double* partial;           // [gridDim.x][nvals] Gram partial sums
+    double scale;              // applied to the data after a complex input (2/N for an inverse transform)
+    int T;                     // rows per CTA (power of two dividing n^2)
+};
+
+__host__ __device__ inline int d1_gram_nvals(int R, int kind) {
+    const int P = R * (R + 1) / 2;
+    return kind == D1_GRAM_PLAIN ? P : kind == D1_GRAM_V ? 3 * P + R : kind == D1_GRAM_E ? 3 * P : 0;
+}
+
+__host__ inline size_t d1_smem_bytes(int n, int RMAX, int T, bool needE, int nmat) {
+    const int M = n / 2;
+    const int LP = (RMAX * T) | 1;
+    size_t b = (size_t)M * LP * 16 + (size_t)M * 16 + (size_t)nmat * 8;
+    if (needE) b += (size_t)3 * T * n * 8;
+    return b + 16;
+}
+
+template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
+__global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
+    constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
+    constexpr bool NEED_E = (OP == D1_OP_NONLIN_E) || (GRAM == D1_GRAM_E);
+    constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : (OP == D1_OP_NONLIN_E || OP == D1_OP_NONLIN_V) ? 3 * RIN * RIN : 0;
+    const int n = a.g.n, M = n >> 1, logM = a.g.log2n - 1, T = a.T;
+    const int nlines = RMAX * T, LP = nlines | 1;
+    const long long q0 = (long long)blockIdx.x * T;          // first row (q = i2 + n*i3)
+    extern __shared__ double2 smem2[];
+    double2* z = smem2;                                       // [M][LP]
+    double2* tw = z + (size_t)M * LP;                         // [M]  exp(-2 pi i k/n), k < n/2
+    double* mat = (double*)(tw + M);                          // [NMAT]
+    double* Et = mat + ((NMAT + 1) & ~1);                     // [3][T][n]
+    const int tid = threadIdx.x, nth = blockDim.x;
+
+    for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
+    for (int i = tid; i < NMAT; i += nth) mat[i] = a.mat[i];
+    if (NEED_E) {
+        const int cnt = T * M;                                // double2 per component
+        for (int i = tid; i < 3 * cnt; i += nth) {
+            const int d = i / cnt, r = i - d * cnt;
+            ((double2*)Et)[i] = ((const double2*)(a.E + (size_t)d * a.g.N))[q0 * M + r];
+        }
+    }
+    if (IN_MODE == D1_IN_CPLX) __syncthreads();               // tw needed by the merge step below
+
+    // ------------------------------------------------------------------ load
+    if (IN_MODE == D1_IN_REAL) {
+        const int cnt = T * M;
+        for (int c = 0; c < RIN; c++) {
+            const double2* src = (const double2*)(a.in_real + (size_t)c * a.g.N) + q0 * M;
+            for (int i = tid; i < cnt; i += nth) {
+                const int t = i / M, j = i - t * M;
+                z[(size_t)j * LP + c * T + t] = src[i];
+            }
+        }
+        __syncthreads();
+    } else {
+        // half-spectrum row Ah[0..M] -> Z[k] = Ze[k] + i Zo[k] at bit-reversed positions, then inverse FFT
+        const int nk = (M >> 1) + 1, nh = a.g.nh;
+        const int items = RIN * T * nk;
+        for (int w = tid; w < items; w += nth) {
+            const int k = w % nk, line = w / nk;
+            const int c = line / T, t = line - c * T;
+            const double2* row = a.in_cplx + (size_t)c * a.g.NC + (q0 + t) * nh;
+            const double2 A = row[k], Bc = cconj(row[M - k]);
+            const double2 ze = make_double2(0.5 * (A.x + Bc.x), 0.5 * (A.y + Bc.y));
+            const double2 df = make_double2(0.5 * (A.x - Bc.x), 0.5 * (A.y - Bc.y));
+            const double2 zo = cmulc(df, tw[k]);                        // 1/2 conj(w^k) (A[k] - conj A[M-k])
+            z[(size_t)brev(k, logM) * LP + line] = make_double2(ze.x - zo.y, ze.y + zo.x);        // Ze + i Zo
+            if (k != 0 && k != M - k)
+                z[(size_t)brev(M - k, logM) * LP + line] = make_double2(ze.x + zo.y, -ze.y + zo.x);  // conj(Ze) + i conj(Zo)
+        }
+        __syncthreads();
+        fft_lines<true>(z, LP, RIN * T, logM, tw, 2);
+    }
+
+    // ------------------------------------------------------------------ point-wise operation across columns
+    if (OP != D1_OP_NONE || IN_MODE == D1_IN_CPLX) {
+        const int items = M * T;
+        for (int w = tid; w < items; w += nth) {
+            const int t = w % T, j = w / T;
+            double2* p = z + (size_t)j * LP + t;
+            double2 x[RIN];
+#pragma unroll
+            for (int c = 0; c < RIN; c++) {
+                x[c] = p[c * T];
+                if (IN_MODE == D1_IN_CPLX) { x[c].x *= a.scale; x[c].y *= a.scale; }
+            }
+            if (OP == D1_OP_NONE) {
+#pragma unroll
+                for (int c = 0; c < RIN; c++) p[c * T] = x[c];
+            } else if (OP == D1_OP_MATVEC) {
+#pragma unroll
+                for (int co = 0; co < ROUT; co++) {
+                    double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int ci = 0; ci < RIN; ci++) {
+                        const double m = mat[ci * ROUT + co];
+                        acc.x = fma(m, x[ci].x, acc.x);
+                        acc.y = fma(m, x[ci].y, acc.y);
+                    }
+                    p[co * T] = acc;
+                }
+            } else {
+                double2 w0, w1, w2;
+                if (OP == D1_OP_NONLIN_E) {
+                    w0 = ((const double2*)Et)[(0 * T + t) * M + j];
+                    w1 = ((const double2*)Et)[(1 * T + t) * M + j];
+                    w2 = ((const double2*)Et)[(2 * T + t) * M + j];
+                } else {
+                    const long long q = q0 + t;
+                    const int i2 = (int)(q % n), i3 = (int)(q / n);
+                    w0 = make_double2(a.g.lo + a.g.h * (2 * j), a.g.lo + a.g.h * (2 * j + 1));
+                    w1 = make_double2(a.g.lo + a.g.h * i2, a.g.lo + a.g.h * i2);
+                    w2 = make_double2(a.g.lo + a.g.h * i3, a.g.lo + a.g.h * i3);
+                }
+#pragma unroll
+                for (int co = 0; co < ROUT; co++) {
+                    double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
+#pragma unroll
+                    for (int ci = 0; ci < RIN; ci++) {
+                        const double m0 = mat[co * RIN + ci], m1 = mat[RIN * RIN + co * RIN + ci],
+                                     m2 = mat[2 * RIN * RIN + co * RIN + ci];
+                        s0.x = fma(m0, x[ci].x, s0.x); s0.y = fma(m0, x[ci].y, s0.y);
+                        s1.x = fma(m1, x[ci].x, s1.x); s1.y = fma(m1, x[ci].y, s1.y);
+                        s2.x = fma(m2, x[ci].x, s2.x); s2.y = fma(m2, x[ci].y, s2.y);
+                    }
+                    p[co * T] = make_double2(fma(w0.x, s0.x, fma(w1.x, s1.x, w2.x * s2.x)),
+                                             fma(w0.y, s0.y, fma(w1.y, s1.y, w2.y * s2.y)));
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ------------------------------------------------------------------ Gram accumulation (ROUT columns)
+    if (GRAM != D1_GRAM_NONE) {
+        constexpr int P = ROUT * (ROUT + 1) / 2;
+        constexpr int NENT = GRAM == D1_GRAM_V ? P + ROUT : P;      // pairs (+ column sums)
+        const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
+        const int items = M * T;
+        double* part = a.partial + (size_t)blockIdx.x * d1_gram_nvals(ROUT, GRAM);
+        for (int e = warp; e < NENT; e += nwarp) {
+            int ca = 0, cb = 0;
+            if (e < P) {                                            // decode pair index -> (ca <= cb)
+                int rem = e;
+                while (rem >= ROUT - ca) { rem -= ROUT - ca; ca++; }
+                cb = ca + rem;
+            } else {
+                ca = cb = e - P;
+            }
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+            for (int w = lane; w < items; w += 32) {
+                const int t = w % T, j = w / T;
+                const double2 za = z[(size_t)j * LP + ca * T + t];
+                if (e >= P) { s0 += za.x + za.y; continue; }
+                const double2 zb = z[(size_t)j * LP + cb * T + t];
+                const double px = za.x * zb.x, py = za.y * zb.y;
+                if (GRAM == D1_GRAM_PLAIN) {
+                    s0 += px + py;
+                } else if (GRAM == D1_GRAM_E) {
+                    const double2 w0 = ((const double2*)Et)[(0 * T + t) * M + j];
+                    const double2 w1 = ((const double2*)Et)[(1 * T + t) * M + j];
+                    const double2 w2 = ((const double2*)Et)[(2 * T + t) * M + j];
+                    s0 = fma(w0.x, px, fma(w0.y, py, s0));
+                    s1 = fma(w1.x, px, fma(w1.y, py, s1));
+                    s2 = fma(w2.x, px, fma(w2.y, py, s2));
+                } else {
+                    const long long q = q0 + t;
+                    const int i2 = (int)(q % n), i3 = (int)(q / n);
+                    const double v1a = a.g.lo + a.g.h * (2 * j), v1b = a.g.lo + a.g.h * (2 * j + 1);
+                    s0 = fma(v1a, px, fma(v1b, py, s0));
+                    s1 = fma(a.g.lo + a.g.h * i2, px + py, s1);
+                    s2 = fma(a.g.lo + a.g.h * i3, px + py, s2);
+                }
+            }
+            s0 = warp_sum(s0);
+            if (GRAM == D1_GRAM_V || GRAM == D1_GRAM_E) { s1 = warp_sum(s1); s2 = warp_sum(s2); }
+            if (lane == 0) {
+                if (GRAM == D1_GRAM_PLAIN) part[e] = s0;
+                else if (e < P) { part[e] = s0; part[P + e] = s1; part[2 * P + e] = s2; }
+                else part[3 * P + (e - P)] = s0;
+            }
+        }
+    }
+
+    // ------------------------------------------------------------------ store
+    if (OUT_MODE & D1_OUT_REAL) {
+        const int cnt = T * M;
+        for (int c = 0; c < ROUT; c++) {
+            double2* dst = (double2*)(a.out_real + (size_t)c * a.g.N) + q0 * M;
+            for (int i = tid; i < cnt; i += nth) {
+                const int t = i / M, j = i - t * M;
+                dst[i] = z[(size_t)j * LP + c * T + t];
+            }
+        }
+    }
+    if (OUT_MODE & D1_OUT_CPLX) {
+        __syncthreads();
+        fft_lines<false>(z, LP, ROUT * T, logM, tw, 2);
+        const int nk = (M >> 1) + 1, nh = a.g.nh;
+        const int items = ROUT * T * nk;
+        for (int w = tid; w < items; w += nth) {
+            const int k = w % nk, line = w / nk;
+            const int c = line / T, t = line - c * T;
+            double2* row = a.out_cplx + (size_t)c * a.g.NC + (q0 + t) * nh;
+            const double2 Zk = z[(size_t)brev(k, logM) * LP + line];
+            const double2 Zm = cconj(z[(size_t)brev((M - k) & (M - 1), logM) * LP + line]);
+            const double2 ze = make_double2(0.5 * (Zk.x + Zm.x), 0.5 * (Zk.y + Zm.y));
+            const double2 zo = make_double2(0.5 * (Zk.y - Zm.y), -0.5 * (Zk.x - Zm.x));      // -(i/2)(Zk - conj Z[M-k])
+            const double2 wz = cmul(zo, tw[k]);
+            row[k] = cadd(ze, wz);
+            if (k != M - k) row[M - k] = cconj(csub(ze, wz));
+        }
+    }
+}
+
+template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
+inline cudaError_t launch_d1(const D1Args& a, cudaStream_t st) {
+    constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
+    constexpr bool NEED_E = (OP == D1_OP_NONLIN_E) || (GRAM == D1_GRAM_E);
+    constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : (OP == D1_OP_NONLIN_E || OP == D1_OP_NONLIN_V) ? 3 * RIN * RIN : 0;
+    auto kern = k_d1<RIN, ROUT, IN_MODE, OP, GRAM, OUT_MODE>;
+    const size_t sm = d1_smem_bytes(a.g.n, RMAX, a.T, NEED_E, (NMAT + 1) & ~1);
+    static size_t configured = 0;
+    if (sm > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e != cudaSuccess) return e;
+        configured = sm;
+    }
+    const unsigned grid = (unsigned)(((long long)a.g.n * a.g.n) / a.T);
+    kern<<<grid, DLR_THREADS, sm, st>>>(a);
+    return cudaGetLastError();
+}
