@@ -111,7 +111,7 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2110_13481_b200 import dlr
+    from paper_2110_13481_b200 import dlr, replicas
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
     torch.cuda.set_device(local_rank)
@@ -124,7 +124,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    X, S, V = inputs.initial_factors(dict(cfg, seed=cfg["seed"] + rank))
+    X, S, V = inputs.initial_factors(replicas.replica_cfg(cfg, rank))
     stream = torch.cuda.Stream(device=dev)
     ctx = dlr.Dlr(dlr.config_from_inputs(cfg), device=dev, stream=stream)
     Xd, Sd, Vd = (torch.from_numpy(np.ascontiguousarray(a.T)).to(dev) for a in (X, S, V))   # column-major on device
@@ -170,10 +170,7 @@ def main():
     h2d = fac_bytes / e2e_steps
     d2h = fac_bytes / e2e_steps + 80
 
-    t = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step, e2e_ms = t.tolist()
+    ms_step, e2e_ms = replicas.max_over_ranks([ms_step, e2e_ms], dev, world)
 
     if rank == 0:
         peak, peak_src = measured_peak()
