@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -39,6 +40,7 @@ struct HostGrid {
     int T1s;              // same for the 1..3 column field passes
     int T3, T3s;          // pencils per CTA in dimension-3 passes
     int T2, NB2, nch2;    // dimension-2 pass tiling
+    int thr1, thr2, thr3; // CTA sizes of the three pass families
 };
 
 struct FlowTab {
@@ -115,15 +117,35 @@ int choose_T3(int n, int RMAX, int nmat) {
     return best;
 }
 
+// Tuning overrides for experiments: DLR_TUNE="t1=8,t3=4,nb2=1,smem2=48,thr1=256,thr2=256,thr3=128" (all optional).
+// Values are validated by the callers (powers of two, shared-memory limits); unknown keys are ignored.
+int tune(const char* key, int dflt) {
+    const char* e = getenv("DLR_TUNE");
+    if (!e) return dflt;
+    const std::string s(e), k = std::string(key) + "=";
+    size_t pos = 0;
+    while ((pos = s.find(k, pos)) != std::string::npos) {
+        if (pos == 0 || s[pos - 1] == ',') return atoi(s.c_str() + pos + k.size());
+        pos += k.size();
+    }
+    return dflt;
+}
+
+int valid_threads(int t) { return (t == 64 || t == 128 || t == 256) ? t : DLR_THREADS; }
+
 void choose_T2(int n, int nh, int& T2, int& NB, int& nch) {
-    int lines = (int)(SMEM_TARGET / ((size_t)n * 16));
+    const size_t target = (size_t)tune("smem2", 48) * 1024;
+    int lines = (int)(target / ((size_t)n * 16));
     if (lines > 255) lines = 255;
     if (lines < 1) lines = 1;
     nch = (nh + lines - 1) / lines;
     T2 = (nh + nch - 1) / nch;
     NB = lines / T2;
+    const int nbo = tune("nb2", 0);
+    if (nbo > 0) NB = nbo;
     if (NB < 1) NB = 1;
     if (NB > 16) NB = 16;
+    while (NB > 1 && d2_smem_bytes(n, T2, NB) > SMEM_MAX) NB--;
 }
 
 struct Carver {
@@ -228,7 +250,13 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     hg.T1s = choose_T1(n, 3, false, 4);
     hg.T3 = choose_T3(n, R, 4 * R * R);
     hg.T3s = choose_T3(n, 3, 0);
+    const int t1 = tune("t1", 0), t3 = tune("t3", 0);
+    if (is_pow2(t1) && t1 <= n * n && d1_smem_bytes(n, R, t1, true, 3 * R * R) <= SMEM_MAX) hg.T1 = t1;
+    if (is_pow2(t3) && t3 <= 16 && d3_smem_bytes(n, R, t3, 4 * R * R) <= SMEM_MAX) hg.T3 = t3;
     choose_T2(n, hg.g.nh, hg.T2, hg.NB2, hg.nch2);
+    hg.thr1 = valid_threads(tune("thr1", DLR_THREADS));
+    hg.thr2 = valid_threads(tune("thr2", DLR_THREADS));
+    hg.thr3 = valid_threads(tune("thr3", DLR_THREADS));
 }
 
 cudaError_t upload_tables(dlr_ctx* c, HostGrid& hg, double lo, double hi) {
@@ -282,21 +310,21 @@ void phase_mark(dlr_ctx* c, const char* name) {
 
 void run_d2(dlr_ctx* c, const HostGrid& hg, double2* data, int ncols, bool inv) {
     D2Args a;
-    a.g = hg.g; a.data = data; a.ncols = ncols; a.T2 = hg.T2; a.NB = hg.NB2; a.nchunks = hg.nch2;
+    a.g = hg.g; a.data = data; a.ncols = ncols; a.T2 = hg.T2; a.NB = hg.NB2; a.nchunks = hg.nch2; a.threads = hg.thr2;
     if (inv) CK(launch_d2<true>(a, c->st)); else CK(launch_d2<false>(a, c->st));
 }
 
 D1Args d1args(const HostGrid& hg) {
     D1Args a;
     memset(&a, 0, sizeof(a));
-    a.g = hg.g; a.T = hg.T1; a.scale = 2.0 / (double)hg.g.N;
+    a.g = hg.g; a.T = hg.T1; a.scale = 2.0 / (double)hg.g.N; a.threads = hg.thr1;
     return a;
 }
 
 D3Args d3args(dlr_ctx* c, const HostGrid& hg) {
     D3Args a;
     memset(&a, 0, sizeof(a));
-    a.g = hg.g; a.T = hg.T3; a.e_scale = c->cfg.e_scale;
+    a.g = hg.g; a.T = hg.T3; a.e_scale = c->cfg.e_scale; a.threads = hg.thr3;
     a.mats = c->ft.p.mats; a.ph1 = c->ft.p.ph1; a.ph2 = c->ft.p.ph2; a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1;
     a.mbuf = c->MB;
     return a;

@@ -39,19 +39,32 @@ __device__ __forceinline__ double2 cconj(double2 a) { return make_double2(a.x, -
 // Forward = decimation in frequency, natural order in -> bit-reversed order out, kernel exp(-2 pi i jk/M).
 // Inverse = the exact transpose: bit-reversed in -> natural out, conjugate twiddles, unnormalised.
 // tw[] holds exp(-2 pi i k / TWN), k < TWN/2, with TWN = M * twmul.
+// Exact unsigned division by a runtime constant without a hardware divide (the streaming loops index with
+// non-power-of-two line counts such as n/2+1):  q = floor(w / d) = umulhi(w, ceil(2^32 / d)), exact for w*d < 2^32.
+struct FastDiv { unsigned d, m; };
+__host__ __device__ inline FastDiv make_fastdiv(unsigned d) {
+    FastDiv f;
+    f.d = d;
+    f.m = d <= 1 ? 0u : (unsigned)((0x100000000ull + d - 1) / d);
+    return f;
+}
+__device__ __forceinline__ unsigned fdiv(unsigned w, FastDiv f) { return f.d == 1 ? w : __umulhi(w, f.m); }
+
 template <int G, bool INV>
-__device__ __forceinline__ void fft_group(double2* s, int LP, int nlines, int M, int lev0, const double2* tw,
+__device__ __forceinline__ void fft_group(double2* s, int LP, FastDiv nl, int logM, int lev0, const double2* tw,
                                           int twmul) {
     constexpr int R = 1 << G;
-    const int B = M >> lev0;          // block size at the first (coarsest) level of the group
-    const int st = B >> G;            // element stride between the R registers
-    const int items = (M >> G) * nlines;
+    const int nlines = (int)nl.d;
+    const int logst = logM - lev0 - G;        // log2 of the element stride between the R registers
+    const int st = 1 << logst;
+    const int logB = logM - lev0;             // block size at the first (coarsest) level of the group
+    const int items = (1 << (logM - G)) * nlines;
     for (int w = threadIdx.x; w < items; w += blockDim.x) {
-        const int line = w % nlines;
-        const int it = w / nlines;
-        const int j = it % st;
-        const int b = it / st;
-        double2* p = s + (size_t)(b * B + j) * LP + line;
+        const int it = (int)fdiv((unsigned)w, nl);
+        const int line = w - it * nlines;
+        const int j = it & (st - 1);
+        const int b = it >> logst;
+        double2* p = s + (size_t)((b << logB) + j) * LP + line;
         double2 a[R];
 #pragma unroll
         for (int q = 0; q < R; q++) a[q] = p[(size_t)q * st * LP];
@@ -110,7 +123,7 @@ template <bool INV>
 __device__ __forceinline__ void fft_lines(double2* s, int LP, int nlines, int logM, const double2* tw, int twmul) {
     int g[3], ng;
     fft_plan(logM, g, ng);
-    const int M = 1 << logM;
+    const FastDiv nl = make_fastdiv((unsigned)nlines);
     int lev[3];
     lev[0] = 0;
     lev[1] = g[0];
@@ -118,9 +131,9 @@ __device__ __forceinline__ void fft_lines(double2* s, int LP, int nlines, int lo
     for (int ii = 0; ii < ng; ii++) {
         const int i = INV ? ng - 1 - ii : ii;
         switch (g[i]) {
-            case 1: fft_group<1, INV>(s, LP, nlines, M, lev[i], tw, twmul); break;
-            case 2: fft_group<2, INV>(s, LP, nlines, M, lev[i], tw, twmul); break;
-            default: fft_group<3, INV>(s, LP, nlines, M, lev[i], tw, twmul); break;
+            case 1: fft_group<1, INV>(s, LP, nl, logM, lev[i], tw, twmul); break;
+            case 2: fft_group<2, INV>(s, LP, nl, logM, lev[i], tw, twmul); break;
+            default: fft_group<3, INV>(s, LP, nl, logM, lev[i], tw, twmul); break;
         }
         __syncthreads();
     }

@@ -25,6 +25,7 @@ struct D1Args {
     double* partial;           // [gridDim.x][nvals] Gram partial sums
     double scale;              // applied to the data after a complex input (2/N for an inverse transform)
     int T;                     // rows per CTA (power of two dividing n^2)
+    int threads;               // CTA size (0 = DLR_THREADS)
 };
 
 __host__ __device__ inline int d1_gram_nvals(int R, int kind) {
@@ -36,32 +37,36 @@ __host__ inline size_t d1_smem_bytes(int n, int RMAX, int T, bool needE, int nma
     const int M = n / 2;
     const int LP = (RMAX * T) | 1;
     size_t b = (size_t)M * LP * 16 + (size_t)M * 16 + (size_t)nmat * 8;
-    if (needE) b += (size_t)3 * T * n * 8;
+    if (needE) b += (size_t)3 * M * (T | 1) * 16;          // E tile as [d][j][t], t padded to odd
     return b + 16;
 }
 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
-__global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
+__global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 ? 2 : 1)) k_d1(const D1Args a) {
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
     constexpr bool NEED_E = (OP == D1_OP_NONLIN_E) || (GRAM == D1_GRAM_E);
     constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : (OP == D1_OP_NONLIN_E || OP == D1_OP_NONLIN_V) ? 3 * RIN * RIN : 0;
-    const int n = a.g.n, M = n >> 1, logM = a.g.log2n - 1, T = a.T;
+    const int n = a.g.n, M = n >> 1, lg = a.g.log2n, logM = lg - 1, T = a.T;
+    const int lt = __ffs(T) - 1, TP = T | 1;                  // log2(T); padded t-stride of the E tile
     const int nlines = RMAX * T, LP = nlines | 1;
     const long long q0 = (long long)blockIdx.x * T;          // first row (q = i2 + n*i3)
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                       // [M][LP]
     double2* tw = z + (size_t)M * LP;                         // [M]  exp(-2 pi i k/n), k < n/2
     double* mat = (double*)(tw + M);                          // [NMAT]
-    double* Et = mat + ((NMAT + 1) & ~1);                     // [3][T][n]
+    double2* Et = (double2*)(mat + ((NMAT + 1) & ~1));        // [3][M][TP] (pairs of grid points along i1)
     const int tid = threadIdx.x, nth = blockDim.x;
 
     for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
     for (int i = tid; i < NMAT; i += nth) mat[i] = a.mat[i];
     if (NEED_E) {
         const int cnt = T * M;                                // double2 per component
-        for (int i = tid; i < 3 * cnt; i += nth) {
-            const int d = i / cnt, r = i - d * cnt;
-            ((double2*)Et)[i] = ((const double2*)(a.E + (size_t)d * a.g.N))[q0 * M + r];
+        for (int d = 0; d < 3; d++) {
+            const double2* src = (const double2*)(a.E + (size_t)d * a.g.N) + q0 * M;
+            for (int i = tid; i < cnt; i += nth) {
+                const int t = i >> logM, j = i & (M - 1);
+                Et[(size_t)(d * M + j) * TP + t] = src[i];
+            }
         }
     }
     if (IN_MODE == D1_IN_CPLX) __syncthreads();               // tw needed by the merge step below
@@ -72,7 +77,7 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
         for (int c = 0; c < RIN; c++) {
             const double2* src = (const double2*)(a.in_real + (size_t)c * a.g.N) + q0 * M;
             for (int i = tid; i < cnt; i += nth) {
-                const int t = i / M, j = i - t * M;
+                const int t = i >> logM, j = i & (M - 1);
                 z[(size_t)j * LP + c * T + t] = src[i];
             }
         }
@@ -80,10 +85,11 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
     } else {
         // half-spectrum row Ah[0..M] -> Z[k] = Ze[k] + i Zo[k] at bit-reversed positions, then inverse FFT
         const int nk = (M >> 1) + 1, nh = a.g.nh;
+        const FastDiv fnk = make_fastdiv((unsigned)nk);
         const int items = RIN * T * nk;
         for (int w = tid; w < items; w += nth) {
-            const int k = w % nk, line = w / nk;
-            const int c = line / T, t = line - c * T;
+            const int line = (int)fdiv((unsigned)w, fnk), k = w - line * nk;
+            const int c = line >> lt, t = line & (T - 1);
             const double2* row = a.in_cplx + (size_t)c * a.g.NC + (q0 + t) * nh;
             const double2 A = row[k], Bc = cconj(row[M - k]);
             const double2 ze = make_double2(0.5 * (A.x + Bc.x), 0.5 * (A.y + Bc.y));
@@ -101,7 +107,7 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
     if (OP != D1_OP_NONE || IN_MODE == D1_IN_CPLX) {
         const int items = M * T;
         for (int w = tid; w < items; w += nth) {
-            const int t = w % T, j = w / T;
+            const int t = w & (T - 1), j = w >> lt;
             double2* p = z + (size_t)j * LP + t;
             double2 x[RIN];
 #pragma unroll
@@ -127,12 +133,12 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
             } else {
                 double2 w0, w1, w2;
                 if (OP == D1_OP_NONLIN_E) {
-                    w0 = ((const double2*)Et)[(0 * T + t) * M + j];
-                    w1 = ((const double2*)Et)[(1 * T + t) * M + j];
-                    w2 = ((const double2*)Et)[(2 * T + t) * M + j];
+                    w0 = Et[(size_t)(0 * M + j) * TP + t];
+                    w1 = Et[(size_t)(1 * M + j) * TP + t];
+                    w2 = Et[(size_t)(2 * M + j) * TP + t];
                 } else {
-                    const long long q = q0 + t;
-                    const int i2 = (int)(q % n), i3 = (int)(q / n);
+                    const int q = (int)q0 + t;
+                    const int i2 = q & (n - 1), i3 = q >> lg;
                     w0 = make_double2(a.g.lo + a.g.h * (2 * j), a.g.lo + a.g.h * (2 * j + 1));
                     w1 = make_double2(a.g.lo + a.g.h * i2, a.g.lo + a.g.h * i2);
                     w2 = make_double2(a.g.lo + a.g.h * i3, a.g.lo + a.g.h * i3);
@@ -174,7 +180,7 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
             }
             double s0 = 0.0, s1 = 0.0, s2 = 0.0;
             for (int w = lane; w < items; w += 32) {
-                const int t = w % T, j = w / T;
+                const int t = w & (T - 1), j = w >> lt;
                 const double2 za = z[(size_t)j * LP + ca * T + t];
                 if (e >= P) { s0 += za.x + za.y; continue; }
                 const double2 zb = z[(size_t)j * LP + cb * T + t];
@@ -182,15 +188,15 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
                 if (GRAM == D1_GRAM_PLAIN) {
                     s0 += px + py;
                 } else if (GRAM == D1_GRAM_E) {
-                    const double2 w0 = ((const double2*)Et)[(0 * T + t) * M + j];
-                    const double2 w1 = ((const double2*)Et)[(1 * T + t) * M + j];
-                    const double2 w2 = ((const double2*)Et)[(2 * T + t) * M + j];
+                    const double2 w0 = Et[(size_t)(0 * M + j) * TP + t];
+                    const double2 w1 = Et[(size_t)(1 * M + j) * TP + t];
+                    const double2 w2 = Et[(size_t)(2 * M + j) * TP + t];
                     s0 = fma(w0.x, px, fma(w0.y, py, s0));
                     s1 = fma(w1.x, px, fma(w1.y, py, s1));
                     s2 = fma(w2.x, px, fma(w2.y, py, s2));
                 } else {
-                    const long long q = q0 + t;
-                    const int i2 = (int)(q % n), i3 = (int)(q / n);
+                    const int q = (int)q0 + t;
+                    const int i2 = q & (n - 1), i3 = q >> lg;
                     const double v1a = a.g.lo + a.g.h * (2 * j), v1b = a.g.lo + a.g.h * (2 * j + 1);
                     s0 = fma(v1a, px, fma(v1b, py, s0));
                     s1 = fma(a.g.lo + a.g.h * i2, px + py, s1);
@@ -213,7 +219,7 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
         for (int c = 0; c < ROUT; c++) {
             double2* dst = (double2*)(a.out_real + (size_t)c * a.g.N) + q0 * M;
             for (int i = tid; i < cnt; i += nth) {
-                const int t = i / M, j = i - t * M;
+                const int t = i >> logM, j = i & (M - 1);
                 dst[i] = z[(size_t)j * LP + c * T + t];
             }
         }
@@ -222,10 +228,11 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d1(const D1Args a) {
         __syncthreads();
         fft_lines<false>(z, LP, ROUT * T, logM, tw, 2);
         const int nk = (M >> 1) + 1, nh = a.g.nh;
+        const FastDiv fnk = make_fastdiv((unsigned)nk);
         const int items = ROUT * T * nk;
         for (int w = tid; w < items; w += nth) {
-            const int k = w % nk, line = w / nk;
-            const int c = line / T, t = line - c * T;
+            const int line = (int)fdiv((unsigned)w, fnk), k = w - line * nk;
+            const int c = line >> lt, t = line & (T - 1);
             double2* row = a.out_cplx + (size_t)c * a.g.NC + (q0 + t) * nh;
             const double2 Zk = z[(size_t)brev(k, logM) * LP + line];
             const double2 Zm = cconj(z[(size_t)brev((M - k) & (M - 1), logM) * LP + line]);
@@ -248,10 +255,12 @@ inline cudaError_t launch_d1(const D1Args& a, cudaStream_t st) {
     static size_t configured = 0;
     if (sm > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         configured = sm;
     }
     const unsigned grid = (unsigned)(((long long)a.g.n * a.g.n) / a.T);
-    kern<<<grid, DLR_THREADS, sm, st>>>(a);
+    kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
     return cudaGetLastError();
 }

@@ -1,6 +1,8 @@
 // Dimension-2 pass: in-place complex FFT (forward: natural -> bit-reversed positions; inverse: the transpose)
 // along k2 of the half spectrum Ah[c][k3'][k2][k1].  Columns are independent here, so a CTA takes NB (column, k3)
 // slabs and a chunk of T2 consecutive k1 (contiguous in memory).
+// Index arithmetic: n is a power of two (shifts); T2 is not (n/2+1 is odd) -> FastDiv; slab decoding is hoisted
+// out of the element loops.
 #pragma once
 #include "common.cuh"
 
@@ -9,6 +11,7 @@ struct D2Args {
     double2* data;       // ncols columns, stride NC
     int ncols;
     int T2, NB, nchunks; // k1 chunk width, slabs per CTA, ceil(nh / T2)
+    int threads;         // CTA size
 };
 
 __host__ inline size_t d2_smem_bytes(int n, int T2, int NB) {
@@ -17,40 +20,46 @@ __host__ inline size_t d2_smem_bytes(int n, int T2, int NB) {
 }
 
 template <bool INV>
-__global__ void __launch_bounds__(DLR_THREADS) k_d2(const D2Args a) {
-    const int n = a.g.n, nh = a.g.nh, T2 = a.T2, NB = a.NB;
+__global__ void __launch_bounds__(DLR_THREADS, 3) k_d2(const D2Args a) {
+    const int n = a.g.n, nh = a.g.nh, lg = a.g.log2n, T2 = a.T2, NB = a.NB;
     const int nlines = T2 * NB, LP = nlines | 1;
     extern __shared__ double2 smem2[];
     double2* z = smem2;
     double2* tw = z + (size_t)n * LP;
     const int tid = threadIdx.x, nth = blockDim.x;
-    const int chunk = blockIdx.x % a.nchunks;
-    const long long slab0 = (long long)(blockIdx.x / a.nchunks) * NB;
-    const long long nslab = (long long)a.ncols * n;
+    const FastDiv fch = make_fastdiv((unsigned)a.nchunks), fT2 = make_fastdiv((unsigned)T2);
+    const int cb = (int)fdiv(blockIdx.x, fch);
+    const int chunk = (int)blockIdx.x - cb * a.nchunks;
+    const int slab0 = cb * NB;
+    const int nslab = a.ncols << lg;
     const int k10 = chunk * T2;
     const int kw = min(T2, nh - k10);
     for (int i = tid; i < n / 2; i += nth) tw[i] = a.g.tw[i];
-    const int items = NB * n * T2;
-    for (int w = tid; w < items; w += nth) {
-        const int ko = w % T2, rest = w / T2;
-        const int k2 = rest % n, sb = rest / n;
-        const long long slab = slab0 + sb;
-        if (ko < kw && slab < nslab) {
-            const long long c = slab / n, k3 = slab % n;
-            z[(size_t)k2 * LP + sb * T2 + ko] = a.data[c * a.g.NC + (k3 * n + k2) * nh + k10 + ko];
-        } else {
-            z[(size_t)k2 * LP + sb * T2 + ko] = make_double2(0.0, 0.0);
+    const int per = n * T2;                                    // elements of one slab chunk (k2, ko)
+    for (int sb = 0; sb < NB; sb++) {
+        const int slab = slab0 + sb;
+        const bool live = slab < nslab;
+        const int c = slab >> lg, k3 = slab & (n - 1);
+        const double2* src = a.data + (size_t)c * a.g.NC + ((size_t)k3 << lg) * nh + k10;
+        double2* dst = z + sb * T2;
+        for (int w = tid; w < per; w += nth) {
+            const int k2 = (int)fdiv((unsigned)w, fT2);
+            const int ko = w - k2 * T2;
+            dst[(size_t)k2 * LP + ko] = (live && ko < kw) ? src[(size_t)k2 * nh + ko] : make_double2(0.0, 0.0);
         }
     }
     __syncthreads();
-    fft_lines<INV>(z, LP, nlines, a.g.log2n, tw, 1);
-    for (int w = tid; w < items; w += nth) {
-        const int ko = w % T2, rest = w / T2;
-        const int k2 = rest % n, sb = rest / n;
-        const long long slab = slab0 + sb;
-        if (ko < kw && slab < nslab) {
-            const long long c = slab / n, k3 = slab % n;
-            a.data[c * a.g.NC + (k3 * n + k2) * nh + k10 + ko] = z[(size_t)k2 * LP + sb * T2 + ko];
+    fft_lines<INV>(z, LP, nlines, lg, tw, 1);
+    for (int sb = 0; sb < NB; sb++) {
+        const int slab = slab0 + sb;
+        if (slab >= nslab) break;
+        const int c = slab >> lg, k3 = slab & (n - 1);
+        double2* out = a.data + (size_t)c * a.g.NC + ((size_t)k3 << lg) * nh + k10;
+        const double2* srcz = z + sb * T2;
+        for (int w = tid; w < per; w += nth) {
+            const int k2 = (int)fdiv((unsigned)w, fT2);
+            const int ko = w - k2 * T2;
+            if (ko < kw) out[(size_t)k2 * nh + ko] = srcz[(size_t)k2 * LP + ko];
         }
     }
 }
@@ -62,11 +71,13 @@ inline cudaError_t launch_d2(const D2Args& a, cudaStream_t st) {
     static size_t configured = 0;
     if (sm > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         configured = sm;
     }
     const long long nslab = (long long)a.ncols * a.g.n;
     const unsigned grid = (unsigned)(a.nchunks * ((nslab + a.NB - 1) / a.NB));
-    kern<<<grid, DLR_THREADS, sm, st>>>(a);
+    kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
     return cudaGetLastError();
 }

@@ -31,6 +31,7 @@ struct D3Args {
     double e_scale;
     int T;                // pencils per CTA
     int skip_store;       // EULER_END: only zero_out is wanted
+    int threads;          // CTA size (0 = DLR_THREADS); must be a multiple of T
 };
 
 __host__ inline size_t d3_smem_bytes(int n, int RMAX, int T, int nmat) {
@@ -63,15 +64,17 @@ __device__ __forceinline__ void phase_c(double2 (&x)[R], const double2* ph) {
 }
 
 template <int RIN, int ROUT, int FOP, bool PGRAM>
-__global__ void __launch_bounds__(DLR_THREADS) k_d3(const D3Args a) {
+__global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 ? 2 : 1)) k_d3(const D3Args a) {
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
     constexpr int R = RIN;
     constexpr int NMAT = (FOP == D3_FWD_STORE || FOP == D3_POISSON || FOP == D3_INV_ONLY) ? 0 : 4 * R * R;
-    const int n = a.g.n, nh = a.g.nh, T = a.T;
+    const int n = a.g.n, nh = a.g.nh, lg = a.g.log2n, T = a.T;
+    const int lt = __ffs(T) - 1;                                 // T is a power of two
     const int LP = (RMAX * T) | 1;
-    const long long plane = (long long)nh * n;
-    const long long p0 = (long long)blockIdx.x * T;
-    const int tw_ = (int)min((long long)T, plane - p0);          // valid pencils in this tile
+    const int plane = nh * n;                                    // pencils per column (<= 129 * 256)
+    const int p0 = (int)blockIdx.x * T;
+    const int tw_ = min(T, plane - p0);                          // valid pencils in this tile
+    const FastDiv fnh = make_fastdiv((unsigned)nh);
     extern __shared__ double2 smem2[];
     double2* z = smem2;
     double2* tw = z + (size_t)n * LP;
@@ -89,8 +92,8 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d3(const D3Args a) {
     {
         const int items = RIN * n * T;
         for (int w = tid; w < items; w += nth) {
-            const int t = w % T, rest = w / T;
-            const int e = rest % n, c = rest / n;
+            const int t = w & (T - 1), rest = w >> lt;
+            const int e = rest & (n - 1), c = rest >> lg;
             z[(size_t)e * LP + c * T + t] =
                 t < tw_ ? a.in[(size_t)c * a.g.NC + (size_t)e * plane + p0 + t] : make_double2(0.0, 0.0);
         }
@@ -110,10 +113,10 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d3(const D3Args a) {
             const int cb = ca + 1 + rem;
             double s0 = 0.0, s1 = 0.0, s2 = 0.0;
             for (int w = lane; w < items; w += 32) {
-                const int t = w % T, e = w / T;
+                const int t = w & (T - 1), e = w >> lt;
                 if (t >= tw_) continue;
-                const long long p = p0 + t;
-                const int k1 = (int)(p % nh), k2 = (int)(p / nh);
+                const int p = p0 + t;
+                const int k2 = (int)fdiv((unsigned)p, fnh), k1 = p - k2 * nh;
                 const double2 za = z[(size_t)e * LP + ca * T + t], zb = z[(size_t)e * LP + cb * T + t];
                 double q = za.y * zb.x - za.x * zb.y;
                 if (k1 != 0 && k1 != nh - 1) q *= 2.0;
@@ -129,11 +132,13 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d3(const D3Args a) {
     // ---- mode-wise operation across the columns
     if (FOP != D3_FWD_STORE) {
         const int items = FOP == D3_INV_ONLY ? 0 : n * T;
+        // blockDim is a multiple of T, so a thread keeps its pencil t (and with it k1, k2) over the whole loop
+        const int t = tid & (T - 1);
+        const int p = p0 + t;
+        const int k2 = (int)fdiv((unsigned)p, fnh), k1 = p - k2 * nh;
         for (int w = tid; w < items; w += nth) {
-            const int t = w % T, e = w / T;
+            const int e = w >> lt;
             if (t >= tw_) continue;
-            const long long p = p0 + t;
-            const int k1 = (int)(p % nh), k2 = (int)(p / nh);
             double2* zp = z + (size_t)e * LP + t;
             if (FOP == D3_POISSON) {
                 const double2 rho = zp[0];
@@ -202,8 +207,8 @@ __global__ void __launch_bounds__(DLR_THREADS) k_d3(const D3Args a) {
     {
         const int items = ROUT * n * T;
         for (int w = tid; w < items; w += nth) {
-            const int t = w % T, rest = w / T;
-            const int e = rest % n, c = rest / n;
+            const int t = w & (T - 1), rest = w >> lt;
+            const int e = rest & (n - 1), c = rest >> lg;
             if (t < tw_) a.out[(size_t)c * a.g.NC + (size_t)e * plane + p0 + t] = z[(size_t)e * LP + c * T + t];
         }
     }
@@ -218,11 +223,13 @@ inline cudaError_t launch_d3(const D3Args& a, cudaStream_t st) {
     static size_t configured = 0;
     if (sm > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         configured = sm;
     }
     const long long plane = (long long)a.g.nh * a.g.n;
     const unsigned grid = (unsigned)((plane + a.T - 1) / a.T);
-    kern<<<grid, DLR_THREADS, sm, st>>>(a);
+    kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
     return cudaGetLastError();
 }
