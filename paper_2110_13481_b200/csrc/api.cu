@@ -58,15 +58,17 @@ struct dlr_ctx {
     dlr_config cfg;
     int R;
     cudaStream_t st, cap_st;
+    cudaStream_t side;            // side branch: the coefficient/eigen kernel overlaps the dim-2/3 passes of its transform
+    cudaEvent_t ev_fork, ev_join;
     const RankOps* ops;
     HostGrid gx, gv;
     // big buffers
     double *X, *V, *S, *Sp;
     double2 *Xh0, *Xh, *Vh, *W, *MB, *Eh;
     double *KL, *Q1, *E;
-    double *partial, *partial2a, *partial2b;
+    double *partial, *partialP, *partial2a;
     // small buffers
-    double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *pvec, *zsum, *mx, *mv, *mres, *esum;
+    double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *zsum, *mx, *mv, *mxp, *mvp, *mres, *esum;
     int* status;
     long long *pix, *piv;
     double* pf;
@@ -206,8 +208,8 @@ size_t carve(dlr_ctx* c, char* base) {
     }
     c->partial_cap = blocks * nvmax;
     c->partial = cv.take<double>(c->partial_cap);
+    c->partialP = cv.take<double>(blocks * (size_t)(3 * R * (R - 1) / 2));   // Parseval sums of the dimension-3 pass
     c->partial2a = cv.take<double>((size_t)DLR_G1 * nvmax);
-    c->partial2b = cv.take<double>((size_t)DLR_G1 * nvmax);
     const int RR = R * R;
     c->S = cv.take<double>(RR); c->Sp = cv.take<double>(RR);
     c->C1 = cv.take<double>(3 * RR); c->C2 = cv.take<double>(3 * RR);
@@ -216,8 +218,9 @@ size_t carve(dlr_ctx* c, char* base) {
     c->TC = cv.take<double>(3 * RR); c->lamC = cv.take<double>(3 * R);
     c->TD = cv.take<double>(3 * RR); c->lamD = cv.take<double>(3 * R);
     c->apply = cv.take<double>(RR); c->Rtot = cv.take<double>(RR);
-    c->pvec = cv.take<double>(R); c->zsum = cv.take<double>(R);
-    c->mx = cv.take<double>(5 * R); c->mv = cv.take<double>(5 * R); c->mres = cv.take<double>(8); c->esum = cv.take<double>(2);
+    c->zsum = cv.take<double>(R);
+    c->mx = cv.take<double>(5 * R); c->mv = cv.take<double>(5 * R); c->mres = cv.take<double>(8);
+    c->mxp = cv.take<double>((size_t)5 * R * DLR_MCH); c->mvp = cv.take<double>((size_t)5 * R * DLR_MCH); c->esum = cv.take<double>(DLR_ECH);
     c->status = cv.take<int>(4);
     c->probe_cap = 4096;
     c->pix = cv.take<long long>(c->probe_cap); c->piv = cv.take<long long>(c->probe_cap); c->pf = cv.take<double>(c->probe_cap);
@@ -340,41 +343,62 @@ int d3_blocks(const HostGrid& hg) { return (int)(((long long)hg.g.nh * hg.g.n + 
 
 // Factor transform: A (real, N x r) -> Ah (half spectrum), accumulating the coefficient sums on the way:
 // kind = 0: none;  1: C coefficients (weights v_i, + rho_tilde);  2: D coefficients (weights E_i).
-void factor_fft(dlr_ctx* c, const HostGrid& hg, const double* A, double2* Ah, int kind, double* M1, double* M2,
-                double* colsum) {
+// With kind != 0: M1 (C1 or D1), its eigen-decomposition (T, lam) and colsum are final when this returns (in stream
+// order); the Parseval sums of the derivative coefficients are left in c->partialP for post(..., do_m2).
+void factor_fft(dlr_ctx* c, const HostGrid& hg, const double* A, double2* Ah, int kind, double* M1, double* colsum,
+                double* T, double* lam) {
     const int R = c->R;
     D1Args a = d1args(hg);
     a.in_real = A; a.out_cplx = Ah; a.E = c->E; a.partial = c->partial;
     CK(c->ops->d1[kind == 0 ? V1_FFT_PLAIN : kind == 1 ? V1_FFT_GRAMV : V1_FFT_GRAME](a, c->st));
-    if (kind) reduce_partials(c, d1_blocks(hg), d1_gram_nvals(R, kind == 1 ? D1_GRAM_V : D1_GRAM_E), c->partial2a);
+    if (kind) {
+        // fork: M1 and its eigen-decomposition need only the Gram sums of the pass above; they run beside the two
+        // remaining passes of the transform (under stream capture this becomes a parallel branch of the step graph)
+        CK(cudaEventRecord(c->ev_fork, c->st));
+        CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+        k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->partial, d1_blocks(hg), R, kind == 1, hg.g.h3, M1, colsum, T, lam);
+        CK(cudaGetLastError());
+        CK(cudaEventRecord(c->ev_join, c->side));
+        c->count_launches -= 3;                     // the three event calls above are not kernel launches
+    }
     run_d2(c, hg, Ah, R, false);
     D3Args b = d3args(c, hg);
-    b.in = Ah; b.out = Ah; b.partial = c->partial;
+    b.in = Ah; b.out = Ah; b.partial = c->partialP;
     CK(c->ops->d3[kind ? V3_FWD_PGRAM : V3_FWD](b, c->st));
     if (kind) {
-        reduce_partials(c, d3_blocks(hg), 3 * R * (R - 1) / 2, c->partial2b);
-        k_finalize_coeff<<<1, 256, 0, c->st>>>(c->partial2a, c->partial2b, R, kind == 1, hg.g.h3, 1.0 / (double)hg.g.N,
-                                               M1, M2, colsum);
-        CK(cudaGetLastError());
+        CK(cudaStreamWaitEvent(c->st, c->ev_join, 0));      // join before anything reads M1, T, lam, colsum
+        c->count_launches -= 1;
     }
 }
 
-void eig3(dlr_ctx* c, const double* M1, double* T, double* lam) {
-    k_eig3<<<1, 96, 0, c->st>>>(M1, c->R, T, lam);
+// The r x r work between two streaming phases, one launch (see k_post).
+struct PostM2 { const HostGrid* hg; double* M2; };
+struct PostS { double* S; double t; };
+struct PostTab { const HostGrid* hg; const double *T, *lam, *Sin; int transS; double sgn, tsub, t3; const double* M2c; double nlsign; };
+void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
+    PostArgs a;
+    memset(&a, 0, sizeof(a));
+    a.R = c->R;
+    if (m2) {
+        a.do_m2 = 1; a.pgram = c->partialP; a.nblocks = d3_blocks(*m2->hg);
+        a.m2scale = m2->hg->g.h3 / (double)m2->hg->g.N; a.M2 = m2->M2;
+    }
+    if (sf) { a.do_s = 1; a.S = sf->S; a.ts = sf->t; a.C1 = c->C1; a.C2 = c->C2; a.D1 = c->D1; a.D2 = c->D2; }
+    if (tb) {
+        a.do_tab = 1; a.Tm = tb->T; a.lam = tb->lam; a.Sin = tb->Sin; a.transS = tb->transS; a.g = tb->hg->g;
+        a.sgn = tb->sgn; a.tsub = tb->tsub; a.t3 = tb->t3; a.M2c = tb->M2c; a.nlsign = tb->nlsign; a.o = c->ft.p;
+    }
+    k_post<<<1, DLR_SMALL_THREADS, 0, c->st>>>(a);
     CK(cudaGetLastError());
 }
 
-void sflow(dlr_ctx* c, double* S, double t) {
-    k_sflow<<<1, 256, 0, c->st>>>(S, c->R, t, c->C1, c->C2, c->D1, c->D2);
-    CK(cudaGetLastError());
-}
-
-// Electric field from rho = A * pvec (pvec already holds the minus sign and weights): eqs. (12)/(13) + Poisson
+// Electric field from rho = A * p (p holds the minus sign and the quadrature weight): eqs. (12)/(13) + Poisson
 // (PAPER.md:180-190):  r2c -> FFT2 -> FFT3, E_hat = -i kt phi_hat, back -> E (3 x N_x real).
-void field(dlr_ctx* c, const double* A) {
+// p = scale * S vec (S != nullptr; vec has element stride vstride) or scale * vec is formed inside the first pass.
+void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int vstride, double scale) {
     const HostGrid& hg = c->gx;
     D1Args a = d1args(hg);
-    a.in_real = A; a.out_cplx = c->Eh; a.mat = c->pvec;
+    a.in_real = A; a.out_cplx = c->Eh; a.rho_S = S; a.rho_vec = vec; a.rho_stride = vstride; a.rho_scale = scale;
     CK(c->ops->d1[V1_RHO](a, c->st));
     run_d2(c, hg, c->Eh, 1, false);
     D3Args b = d3args(c, hg);
@@ -390,26 +414,19 @@ void field(dlr_ctx* c, const double* A) {
 // (transS: S = R^T for the L step, Fig. 1 line 40 transpose_inplace).
 // The Gram sums of KL must already be in c->partial (written by the pass that produced KL).
 void qr(dlr_ctx* c, const HostGrid& hg, double* basis, double* Sout, int transS) {
-    const int R = c->R, P = R * (R + 1) / 2;
+    const int R = c->R;
     const double shift = 64.0 * R * 2.220446049250313e-16;
     const double osc = 1.0 / sqrt(hg.g.h3), ssc = sqrt(hg.g.h3);
     double* src[3] = {c->KL, c->Q1, c->KL};
     double* dst[3] = {c->Q1, c->KL, basis};
     for (int stage = 0; stage < 3; stage++) {
-        reduce_partials(c, d1_blocks(hg), P, c->partial2a);
-        k_chol_stage<<<1, 32, 0, c->st>>>(c->partial2a, R, stage, stage == 2, shift, osc, ssc, transS, c->apply, c->Rtot,
-                                          Sout, c->status);
+        k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->partial, d1_blocks(hg), R, stage, stage == 2, shift, osc, ssc,
+                                                          transS, c->apply, c->Rtot, Sout, c->status);
         CK(cudaGetLastError());
         D1Args a = d1args(hg);
         a.in_real = src[stage]; a.out_real = dst[stage]; a.mat = c->apply; a.partial = c->partial;
         CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
     }
-}
-
-void flow_tables(dlr_ctx* c, const HostGrid& hg, const double* T, const double* lam, const double* Sin, int transS,
-                 double sgn, double tsub, double t3, const double* M2c, double nlsign) {
-    k_flow_tables<<<1, 256, 0, c->st>>>(T, lam, Sin, transS, c->R, hg.g, sgn, tsub, t3, M2c, nlsign, c->ft.p);
-    CK(cudaGetLastError());
 }
 
 // K- or L-flow of section 4 starting from the spectrum `spec` of the basis (the product with the
@@ -448,45 +465,43 @@ void flow(dlr_ctx* c, const HostGrid& hg, const double2* spec, bool is_L, int or
     CK(ops->d1[V1_INV_GRAM](o, c->st));
 }
 
-void rho_vec(dlr_ctx* c, const double* S, const double* vec, int use_S, double scale) {
-    k_rho_vec<<<1, 32, 0, c->st>>>(S, vec, c->R, use_S, scale, c->pvec);
-    CK(cudaGetLastError());
-}
-
 // one step, issued on c->st (directly or under stream capture)
 void issue_step(dlr_ctx* c, double tau) {
     const int order = c->cfg.order;
     const double tp = order == 2 ? 0.5 * tau : tau;     // step size of the Algorithm-1 part
     const HostGrid &gx = c->gx, &gv = c->gv;
     double* Sp = order == 2 ? c->Sp : c->S;             // the predictor of Algorithm 2 works on a scratch S
+    const PostM2 m2C{&gv, c->C2}, m2D{&gx, c->D2};
     phase_mark(c, "start");
     // ---- Algorithm 1, line 1: C coefficients from V0 (kept from the previous step's line 10 when valid)
     if (!c->vh_valid) {
-        factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->C2, c->rho_t);
-        eig3(c, c->C1, c->TC, c->lamC);
+        factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->rho_t, c->TC, c->lamC);
+        post(c, &m2C, nullptr, nullptr);
     }
     phase_mark(c, "C coefficients (V0)");
     // ---- line 2: K0 = X0 S0, kept as the spectrum of X0 (the product with S0 is folded into the flow)
-    factor_fft(c, gx, c->X, c->Xh0, 0, nullptr, nullptr, nullptr);
+    factor_fft(c, gx, c->X, c->Xh0, 0, nullptr, nullptr, nullptr, nullptr);
     // ---- line 3: E0 from K0 and V0, eq. (12): rho = -X0 (S0 rho_tilde)
-    rho_vec(c, c->S, c->rho_t, 1, -1.0);
-    field(c, c->X);
+    field(c, c->X, c->S, c->rho_t, 1, -1.0);
     phase_mark(c, "electric field E0");
     // ---- line 4: K step (Lie, exponential Euler) of length tp with E0;  line 5: QR -> X1, S1
-    flow_tables(c, gx, c->TC, c->lamC, c->S, 0, -1.0, tp, tp, c->C2, 1.0);
+    {
+        const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, tp, tp, c->C2, 1.0};
+        post(c, nullptr, nullptr, &tb);
+    }
     flow(c, gx, c->Xh0, false, 1, false);
     phase_mark(c, "K step (predictor)");
     qr(c, gx, c->X, Sp, 0);
     phase_mark(c, "QR K (predictor)");
-    // ---- line 6: D coefficients from X1 and E0
-    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, c->D2, nullptr);
-    eig3(c, c->D1, c->TD, c->lamD);
+    // ---- line 6: D coefficients from X1 and E0;  line 7: S step;  lines 8-9: L0 = V0 S2^T, tables of the L step
+    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, nullptr, c->TD, c->lamD);
     phase_mark(c, "D coefficients (predictor)");
-    // ---- line 7: S step
-    sflow(c, Sp, tp);
+    {
+        const PostS sf{Sp, tp};
+        const PostTab tb{&gv, c->TD, c->lamD, Sp, 1, +1.0, tp, tp, c->D2, -1.0};
+        post(c, &m2D, &sf, &tb);
+    }
     phase_mark(c, "S step (predictor)");
-    // ---- lines 8-9: L0 = V0 S2^T, L step with E0
-    flow_tables(c, gv, c->TD, c->lamD, Sp, 1, +1.0, tp, tp, c->D2, -1.0);
     if (order == 1) {
         flow(c, gv, c->Vh, true, 1, false);
         phase_mark(c, "L step");
@@ -498,35 +513,42 @@ void issue_step(dlr_ctx* c, double tau) {
     flow(c, gv, c->Vh, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
     phase_mark(c, "L step (predictor)");
     // ---- Algorithm 2, line 2: E^{1/2} from X1 and L1, eq. (13)
-    rho_vec(c, c->S, c->zsum, 0, -gv.g.h3);
-    field(c, c->X);
+    field(c, c->X, nullptr, c->zsum, 1, -gv.g.h3);
     phase_mark(c, "electric field E1/2");
     // ---- line 3: K step (Strang, ETD2RK) of length tau/2 from K0 = X0 S0 with E^{1/2};  line 4: QR -> X2, S3
-    flow_tables(c, gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0);
+    {
+        const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0};
+        post(c, nullptr, nullptr, &tb);
+    }
     flow(c, gx, c->Xh0, false, 2, false);
     phase_mark(c, "first K step");
     qr(c, gx, c->X, c->S, 0);
     phase_mark(c, "QR K (first)");
-    // ---- line 5: D coefficients from X2 and E^{1/2};  line 6: S step
-    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, c->D2, nullptr);
-    eig3(c, c->D1, c->TD, c->lamD);
+    // ---- line 5: D coefficients from X2 and E^{1/2};  line 6: S step;  tables of the L step (L = V0 S4^T)
+    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, nullptr, c->TD, c->lamD);
     phase_mark(c, "D coefficients");
-    sflow(c, c->S, 0.5 * tau);
+    {
+        const PostS sf{c->S, 0.5 * tau};
+        const PostTab tb{&gv, c->TD, c->lamD, c->S, 1, +1.0, 0.5 * tau, tau, c->D2, -1.0};
+        post(c, &m2D, &sf, &tb);
+    }
     phase_mark(c, "first S step");
-    // ---- lines 7-9: L = V0 S4^T, L step (Strang) of length tau, QR -> V1, S5 = R^T
-    flow_tables(c, gv, c->TD, c->lamD, c->S, 1, +1.0, 0.5 * tau, tau, c->D2, -1.0);
+    // ---- lines 7-9: L step (Strang) of length tau, QR -> V1, S5 = R^T
     flow(c, gv, c->Vh, true, 2, false);
     phase_mark(c, "L step");
     qr(c, gv, c->V, c->S, 1);
     phase_mark(c, "QR L");
-    // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step
-    factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->C2, c->rho_t);
-    eig3(c, c->C1, c->TC, c->lamC);
+    // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step;
+    //      tables of the second K step (K3 = X2 S6; the spectrum of X2 is in Xh)
+    factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->rho_t, c->TC, c->lamC);
     phase_mark(c, "C coefficients");
-    sflow(c, c->S, 0.5 * tau);
+    {
+        const PostS sf{c->S, 0.5 * tau};
+        const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0};
+        post(c, &m2C, &sf, &tb);
+    }
     phase_mark(c, "second S step");
-    // ---- lines 12-14: K3 = X2 S6 (spectrum of X2 is in Xh), K step (Strang) of length tau/2, QR -> X3, S7
-    flow_tables(c, gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0);
+    // ---- lines 12-14: K step (Strang) of length tau/2, QR -> X3, S7
     flow(c, gx, c->Xh, false, 2, false);
     phase_mark(c, "second K step");
     qr(c, gx, c->X, c->S, 0);
@@ -593,7 +615,10 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev == 0) { delete c; return DLR_ERR_CUDA; }
     e = cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
+    if (e != cudaSuccess) { dlr_destroy(c); return DLR_ERR_CUDA; }
     e = upload_tables(c, c->gx, cfg->x_lo[0], cfg->x_hi[0]);
     if (e == cudaSuccess) e = upload_tables(c, c->gv, cfg->v_lo[0], cfg->v_hi[0]);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->status, 0, 4 * sizeof(int), c->st);
@@ -607,6 +632,9 @@ void dlr_destroy(dlr_ctx* c) {
     if (!c) return;
     if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->cap_st) cudaStreamDestroy(c->cap_st);
+    if (c->side) cudaStreamDestroy(c->side);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (auto& p : c->phases) cudaEventDestroy(p.ev);
     delete c;
 }
@@ -732,18 +760,18 @@ int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* prob
     if (!c->has_state) return DLR_ERR_NO_STATE;
     if (n_probe < 0 || n_probe > c->probe_cap || (n_probe > 0 && (!probe_ix || !probe_iv || !f_probe))) return DLR_ERR_INVALID;
     const int R = c->R;
-    k_colmoments<<<R, 1024, 0, c->st>>>(c->X, c->gx.g, c->mx);
+    k_colmoments<<<dim3(R, DLR_MCH), 256, 0, c->st>>>(c->X, c->gx.g, c->mxp);
     CK(cudaGetLastError());
-    k_colmoments<<<R, 1024, 0, c->st>>>(c->V, c->gv.g, c->mv);
+    k_colmoments<<<dim3(R, DLR_MCH), 256, 0, c->st>>>(c->V, c->gv.g, c->mvp);
     CK(cudaGetLastError());
-    k_moments_final<<<1, 32, 0, c->st>>>(c->mx, c->mv, c->S, R, c->gx.g.h3, c->gv.g.h3, c->mres);
+    k_colmoments_sum<<<1, 256, 0, c->st>>>(c->mxp, c->mvp, R, c->mx, c->mv);
     CK(cudaGetLastError());
     // electric energy: E from eq. (12) on the current factors.  rho_tilde = h_v^3 V^T 1 = h_v^3 * mv[:,0]
     // (uses the scratch field buffers; the step does not depend on them across steps)
-    k_rho_vec<<<1, 32, 0, c->st>>>(c->S, c->mv, R, 2, -c->gv.g.h3, c->pvec);
+    field(c, c->X, c->S, c->mv, 5, -c->gv.g.h3);
+    k_sumsq<<<DLR_ECH, 256, 0, c->st>>>(c->E, 3 * c->gx.g.N, c->esum);
     CK(cudaGetLastError());
-    field(c, c->X);
-    k_sumsq<<<1, 1024, 0, c->st>>>(c->E, 3 * c->gx.g.N, c->esum);
+    k_moments_final<<<1, 32, 0, c->st>>>(c->mx, c->mv, c->S, R, c->gx.g.h3, c->gv.g.h3, c->esum, c->mres);
     CK(cudaGetLastError());
     if (n_probe > 0) {
         cudaError_t e = cudaMemcpyAsync(c->pix, probe_ix, n_probe * sizeof(int64_t), cudaMemcpyHostToDevice, c->st);
@@ -752,10 +780,9 @@ int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* prob
         k_probes<<<(n_probe + 127) / 128, 128, 0, c->st>>>(c->X, c->S, c->V, c->gx.g.N, c->gv.g.N, R, n_probe, c->pix, c->piv, c->pf);
         CK(cudaGetLastError());
     }
-    double res[8], es[2];
+    double res[8];
     int st[4];
     cudaError_t e = cudaMemcpyAsync(res, c->mres, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(es, c->esum, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(st, c->status, 4 * sizeof(int), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess && n_probe > 0) e = cudaMemcpyAsync(f_probe, c->pf, n_probe * sizeof(double), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
@@ -766,7 +793,7 @@ int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* prob
     out->kinetic_energy = res[4];
     out->s_fro = res[5];
     out->nonfinite = res[6] != 0.0;
-    out->electric_energy = 0.5 * c->gx.g.h3 * es[0];
+    out->electric_energy = 0.5 * c->gx.g.h3 * res[7];
     out->qr_fallbacks = st[0];
     return DLR_OK;
 }

@@ -26,6 +26,13 @@ struct D1Args {
     double scale;              // applied to the data after a complex input (2/N for an inverse transform)
     int T;                     // rows per CTA (power of two dividing n^2)
     int threads;               // CTA size (0 = DLR_THREADS)
+    // charge-density vector of eqs. (12)/(13) (ROUT = 1, MATVEC): if rho_vec != nullptr the CTA forms
+    // mat[i] = rho_scale * sum_j rho_S[i + RIN j] rho_vec[j * rho_stride]   (rho_S column-major r x r), or
+    // mat[i] = rho_scale * rho_vec[i * rho_stride] when rho_S == nullptr, instead of reading `mat`.
+    const double* rho_S;
+    const double* rho_vec;
+    int rho_stride;
+    double rho_scale;
 };
 
 __host__ __device__ inline int d1_gram_nvals(int R, int kind) {
@@ -58,7 +65,18 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     const int tid = threadIdx.x, nth = blockDim.x;
 
     for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
-    for (int i = tid; i < NMAT; i += nth) mat[i] = a.mat[i];
+    if (OP == D1_OP_MATVEC && ROUT == 1 && a.rho_vec != nullptr) {
+        for (int i = tid; i < RIN; i += nth) {
+            double sacc = 0.0;
+            if (a.rho_S != nullptr)
+                for (int j = 0; j < RIN; j++) sacc = fma(a.rho_S[i + RIN * j], a.rho_vec[(size_t)j * a.rho_stride], sacc);
+            else
+                sacc = a.rho_vec[(size_t)i * a.rho_stride];
+            mat[i] = a.rho_scale * sacc;
+        }
+    } else {
+        for (int i = tid; i < NMAT; i += nth) mat[i] = a.mat[i];
+    }
     if (NEED_E) {
         const int cnt = T * M;                                // double2 per component
         for (int d = 0; d < 3; d++) {

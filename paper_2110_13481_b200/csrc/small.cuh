@@ -8,6 +8,7 @@
 
 #define DLR_G1 32          // number of second-level partial rows
 #define DLR_RMAXS 24       // largest rank the small kernels are dimensioned for
+#define DLR_SMALL_THREADS 512   // CTA size of the single-CTA r x r kernels (also the width of their inline reductions)
 
 // ---------------------------------------------------------------------------------------------------------
 // two-level deterministic reduction of per-CTA partial sums: out[g][v] = sum_{b in slice g} partial[b][v]
@@ -28,91 +29,133 @@ __device__ __forceinline__ double sum_g1(const double* p2, int nvals, int v) {
     return s;
 }
 
-// ---------------------------------------------------------------------------------------------------------
-// coefficients from the reduced Gram sums.  gram: [DLR_G1][3P (+R)] (real-space, weights v_i or E_i),
-// pgram: [DLR_G1][3 P2] (Parseval sums for the derivative coefficients).
-//   M1_i = h^3 A^T diag(w_i) A (symmetric), M2_i = h^3 A^T d_i A (antisymmetric),
-//   colsum = h^3 A^T 1 (rho_tilde of eq. (12)) if with_colsum.
-__global__ void k_finalize_coeff(const double* gram, const double* pgram, int R, int with_colsum, double h3,
-                                 double invN, double* M1, double* M2, double* colsum) {
-    const int P = R * (R + 1) / 2, P2 = R * (R - 1) / 2;
-    const int nv1 = 3 * P + (with_colsum ? R : 0), nv2 = 3 * P2;
-    for (int idx = threadIdx.x; idx < 3 * R * R; idx += blockDim.x) {
-        const int d = idx / (R * R), a = (idx / R) % R, b = idx % R;
-        const int lo = min(a, b), hi = max(a, b);
-        const int pe = lo * R - lo * (lo - 1) / 2 + (hi - lo);           // pair index of (lo <= hi)
-        M1[idx] = h3 * sum_g1(gram, nv1, d * P + pe);
-        double v = 0.0;
-        if (a != b) {
-            const int pe2 = lo * (R - 1) - lo * (lo - 1) / 2 + (hi - lo - 1);
-            v = h3 * invN * sum_g1(pgram, nv2, d * P2 + pe2);
-            if (a > b) v = -v;
+// CTA-wide deterministic reduction of per-CTA partial rows, done by the consumer kernel itself (no separate
+// reduction launch):  out[v] = sum_b partial[b * stride + off + v],  v < nvals <= blockDim.x.
+// Thread (g, v) sums the rows b = g, g+G, ... (coalesced in v), then the G group sums are added in fixed order.
+// out: shared [nvals]; tmp: shared [blockDim.x].  Ends with a __syncthreads().
+__device__ __forceinline__ void cta_reduce_rows(const double* __restrict__ partial, int nblocks, int stride, int off,
+                                                int nvals, double* out, double* tmp) {
+    const int nth = blockDim.x, tid = threadIdx.x;
+    const int G = nth / nvals;                     // >= 1
+    const int g = tid / nvals, v = tid - g * nvals;
+    if (g < G) {
+        const double* p = partial + off + v;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        int b = g;
+        for (; b + 3 * G < nblocks; b += 4 * G) {
+            s0 += p[(size_t)b * stride];
+            s1 += p[(size_t)(b + G) * stride];
+            s2 += p[(size_t)(b + 2 * G) * stride];
+            s3 += p[(size_t)(b + 3 * G) * stride];
         }
-        M2[idx] = v;
+        for (; b < nblocks; b += G) s0 += p[(size_t)b * stride];
+        tmp[g * nvals + v] = (s0 + s1) + (s2 + s3);
     }
-    if (with_colsum)
-        for (int c = threadIdx.x; c < R; c += blockDim.x) colsum[c] = h3 * sum_g1(gram, nv1, 3 * P + c);
+    __syncthreads();
+    if (tid < nvals) {
+        double s = 0.0;
+        for (int gg = 0; gg < G; gg++) s += tmp[gg * nvals + tid];
+        out[tid] = s;
+    }
+    __syncthreads();
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// cyclic Jacobi eigen-decomposition of three symmetric r x r matrices (one warp each): Msym = T diag(lam) T^T
-// (PAPER.md:260).  The input is symmetrised first (reading R5).
-__global__ void k_eig3(const double* M1, int R, double* Tout, double* lam) {
-    __shared__ double As[3][DLR_RMAXS][DLR_RMAXS + 1];
-    __shared__ double Ts[3][DLR_RMAXS][DLR_RMAXS + 1];
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (w >= 3) return;
-    const double* Min = M1 + (size_t)w * R * R;
-    double(*A)[DLR_RMAXS + 1] = As[w];
-    double(*T)[DLR_RMAXS + 1] = Ts[w];
-    for (int i = lane; i < R; i += 32)
-        for (int j = 0; j < R; j++) {
-            A[i][j] = 0.5 * (Min[i * R + j] + Min[j * R + i]);
-            T[i][j] = i == j ? 1.0 : 0.0;
-        }
-    __syncwarp();
-    double nrm = 0.0;
-    for (int i = lane; i < R; i += 32)
-        for (int j = 0; j < R; j++) nrm += A[i][j] * A[i][j];
-    nrm = sqrt(warp_sum(nrm));
-    for (int sweep = 0; sweep < 60; sweep++) {
-        double off = 0.0;
-        for (int i = lane; i < R; i += 32)
-            for (int j = i + 1; j < R; j++) off += A[i][j] * A[i][j];
-        off = sqrt(warp_sum(off));
-        if (off <= 1e-16 * nrm || off == 0.0) break;
-        for (int p = 0; p < R - 1; p++)
-            for (int q = p + 1; q < R; q++) {
-                const double apq = A[p][q];
-                if (fabs(apq) <= 1e-20 * nrm) continue;          // warp-uniform
-                const double theta = (A[q][q] - A[p][p]) / (2.0 * apq);
-                const double t = fabs(theta) > 1e150 ? 0.5 / theta
-                                                     : copysign(1.0, theta) / (fabs(theta) + sqrt(theta * theta + 1.0));
-                const double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
-                __syncwarp();
-                if (lane < R) {
-                    const double aip = A[lane][p], aiq = A[lane][q];
-                    A[lane][p] = c * aip - s * aiq;
-                    A[lane][q] = s * aip + c * aiq;
-                    const double tip = T[lane][p], tiq = T[lane][q];
-                    T[lane][p] = c * tip - s * tiq;
-                    T[lane][q] = s * tip + c * tiq;
-                }
-                __syncwarp();
-                if (lane < R) {
-                    const double api = A[p][lane], aqi = A[q][lane];
-                    A[p][lane] = c * api - s * aqi;
-                    A[q][lane] = s * api + c * aqi;
-                }
-                __syncwarp();
-                if (lane == 0) { A[p][q] = 0.0; A[q][p] = 0.0; }
-                __syncwarp();
-            }
+// First half of a coefficient set + its eigen-decompositions, one CTA per direction d (grid = 3):
+//   M1_d = h^3 A^T diag(w_d) A from the real-space Gram partial sums of the dimension-1 pass,
+//   colsum = h^3 A^T 1 (rho_tilde of eq. (12); CTA 0, if with_colsum),
+//   M1_d (symmetrised, reading R5) = T diag(lam) T^T by cyclic Jacobi with ROUND-ROBIN pair ordering:
+//   every round rotates R/2 disjoint pairs at once, A <- J^T A J and T <- T J entry-wise from the previous
+//   buffer (two barriers per round instead of a serial chain of R(R-1)/2 rotations per sweep).
+// partial: [nblocks][3P (+R)], entry e of direction d at d*P + e, column sums at 3P + c.
+#define DLR_EIG_THREADS 256
+__global__ void __launch_bounds__(DLR_EIG_THREADS)
+k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double h3, double* M1, double* colsum,
+             double* Tout, double* lam) {
+    __shared__ double As[2][DLR_RMAXS][DLR_RMAXS + 1], Ts[2][DLR_RMAXS][DLR_RMAXS + 1];
+    __shared__ double red[DLR_RMAXS * (DLR_RMAXS + 1) / 2], tmp[DLR_EIG_THREADS];
+    __shared__ double alpha[DLR_RMAXS], beta[DLR_RMAXS], sq[DLR_RMAXS];
+    __shared__ int part[DLR_RMAXS];
+    __shared__ double s_nrm2, s_off2;
+    const int d = blockIdx.x, tid = threadIdx.x, nth = blockDim.x;
+    const int P = R * (R + 1) / 2, nv = 3 * P + (with_colsum ? R : 0), RR = R * R;
+    if (d == 0 && with_colsum) {
+        cta_reduce_rows(partial, nblocks, nv, 3 * P, R, red, tmp);
+        if (tid < R) colsum[tid] = h3 * red[tid];
+        __syncthreads();
     }
-    __syncwarp();
-    for (int i = lane; i < R; i += 32) {
-        lam[w * R + i] = A[i][i];
-        for (int j = 0; j < R; j++) Tout[(size_t)w * R * R + i * R + j] = T[i][j];
+    cta_reduce_rows(partial, nblocks, nv, d * P, P, red, tmp);
+    for (int idx = tid; idx < RR; idx += nth) {
+        const int i = idx / R, j = idx - i * R;
+        const int lo = min(i, j), hi = max(i, j);
+        const double v = h3 * red[lo * R - lo * (lo - 1) / 2 + (hi - lo)];     // symmetric by construction
+        As[0][i][j] = v;
+        Ts[0][i][j] = i == j ? 1.0 : 0.0;
+        M1[(size_t)d * RR + idx] = v;
+    }
+    __syncthreads();
+    if (tid < 32) {
+        double nr = 0.0;
+        for (int idx = tid; idx < RR; idx += 32) { const double v = As[0][idx / R][idx % R]; nr += v * v; }
+        nr = warp_sum(nr);
+        if (tid == 0) s_nrm2 = nr;
+    }
+    __syncthreads();
+    const double nrm2 = s_nrm2;
+    const int m = R + (R & 1), half = m >> 1;
+    int cur = 0;
+    for (int sweep = 0; sweep < 40; sweep++) {
+        double myoff = 0.0;                                     // sum of apq^2 met by this thread's pairs
+        for (int r = 0; r < m - 1; r++) {
+            if (tid < half) {
+                int p = tid == 0 ? m - 1 : (r + tid) % (m - 1);
+                int q = (r + m - 1 - tid) % (m - 1);
+                if (p > q) { const int t = p; p = q; q = t; }
+                if (q >= R) {                                   // paired with the padding index: untouched
+                    alpha[p] = 1.0; beta[p] = 0.0; part[p] = p;
+                } else {
+                    const double apq = As[cur][p][q];
+                    myoff += apq * apq;
+                    double c = 1.0, sn = 0.0;
+                    if (apq * apq > 1e-40 * nrm2) {
+                        const double theta = (As[cur][q][q] - As[cur][p][p]) / (2.0 * apq);
+                        const double t = fabs(theta) > 1e150 ? 0.5 / theta
+                                                             : copysign(1.0, theta) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                        c = 1.0 / sqrt(t * t + 1.0);
+                        sn = t * c;
+                    }
+                    alpha[p] = c; beta[p] = -sn; part[p] = q;   // new column p = c a_p - s a_q
+                    alpha[q] = c; beta[q] = sn; part[q] = p;    // new column q = s a_p + c a_q
+                }
+            }
+            __syncthreads();
+            const int nxt = cur ^ 1;
+            for (int idx = tid; idx < RR; idx += nth) {
+                const int i = idx / R, j = idx - i * R;
+                const int pi = part[i], pj = part[j];
+                const double ai = alpha[i], bi = beta[i], aj = alpha[j], bj = beta[j];
+                double v = ai * (aj * As[cur][i][j] + bj * As[cur][i][pj]) + bi * (aj * As[cur][pi][j] + bj * As[cur][pi][pj]);
+                if (pi == j && i != j && (bi != 0.0)) v = 0.0;  // the rotated pair's off-diagonal entry is annihilated
+                As[nxt][i][j] = v;
+                Ts[nxt][i][j] = aj * Ts[cur][i][j] + bj * Ts[cur][i][pj];
+            }
+            cur = nxt;
+            __syncthreads();
+        }
+        if (tid < DLR_RMAXS) sq[tid] = tid < half ? myoff : 0.0;
+        __syncthreads();
+        if (tid == 0) {
+            double o = 0.0;
+            for (int k = 0; k < half; k++) o += sq[k];
+            s_off2 = o;
+        }
+        __syncthreads();
+        if (s_off2 <= 1e-32 * nrm2) break;                     // off-diagonal norm met in this sweep <= 1e-16 ||A||_F
+    }
+    for (int idx = tid; idx < RR; idx += nth) {
+        const int i = idx / R, j = idx - i * R;
+        Tout[(size_t)d * RR + idx] = Ts[cur][i][j];
+        if (i == j) lam[d * R + i] = As[cur][i][i];
     }
 }
 
@@ -155,8 +198,9 @@ struct FlowTabPtrs {
     double2 *ph1, *ph2, *ez, *f1, *f2a, *f2b;
 };
 
-__global__ void k_flow_tables(const double* Tm, const double* lam, const double* Sin, int transS, int R, GridDev g,
-                              double sgn, double tsub, double t3, const double* M2c, double nlsign, FlowTabPtrs o) {
+__device__ __forceinline__ void dev_flow_tables(const double* Tm, const double* lam, const double* Sin, int transS,
+                                                int R, const GridDev& g, double sgn, double tsub, double t3,
+                                                const double* M2c, double nlsign, const FlowTabPtrs& o) {
     const double* T1 = Tm;
     const double* T2 = Tm + R * R;
     const double* T3 = Tm + 2 * R * R;
@@ -207,10 +251,17 @@ __global__ void k_flow_tables(const double* Tm, const double* lam, const double*
 
 // ---------------------------------------------------------------------------------------------------------
 // S step: one classical RK4 step of eq. (10):  dS/dt = sum_i D2_i S C1_i^T - D1_i S C2_i^T
-__global__ void k_sflow(double* S, int R, double t, const double* C1, const double* C2, const double* D1,
-                        const double* D2) {
-    __shared__ double Sc[DLR_RMAXS * DLR_RMAXS], Y[DLR_RMAXS * DLR_RMAXS], Kacc[DLR_RMAXS * DLR_RMAXS];
-    __shared__ double Pm[3][DLR_RMAXS * DLR_RMAXS], Qm[3][DLR_RMAXS * DLR_RMAXS];
+#define DLR_RR 400          // r^2 for the largest supported rank (20)
+struct SflowScratch {
+    double Sc[DLR_RR], Y[DLR_RR], Kacc[DLR_RR], Pm[3][DLR_RR], Qm[3][DLR_RR];
+};
+__device__ __forceinline__ void dev_sflow(double* S, int R, double t, const double* C1, const double* C2,
+                                          const double* D1, const double* D2, SflowScratch& sc) {
+    double (&Sc)[DLR_RR] = sc.Sc;
+    double (&Y)[DLR_RR] = sc.Y;
+    double (&Kacc)[DLR_RR] = sc.Kacc;
+    double (&Pm)[3][DLR_RR] = sc.Pm;
+    double (&Qm)[3][DLR_RR] = sc.Qm;
     const int RR = R * R;
     for (int i = threadIdx.x; i < RR; i += blockDim.x) { Sc[i] = S[i]; Y[i] = S[i]; Kacc[i] = 0.0; }
     __syncthreads();
@@ -248,146 +299,202 @@ __global__ void k_sflow(double* S, int R, double t, const double* C1, const doub
         __syncthreads();
     }
     for (int i = threadIdx.x; i < RR; i += blockDim.x) S[i] = Sc[i] + (t / 6.0) * Kacc[i];
+    __syncthreads();
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// One stage of (shifted) CholeskyQR on the reduced Gram sums (one warp).
-//   gram: [DLR_G1][P] upper pairs of A^T A.   stage 0 adds `shift` to the unit-diagonal scaled Gram matrix.
-//   apply[ci][co] : matrix for the next A*Mat pass (= D U^-1, times out_scale on the last stage)
-//   Rtot (row-major, upper triangular) accumulates R_stage * Rtot.
-//   On the last stage the coupling matrix is written: Sout column-major = Rtot*s_scale (transS=0) or its transpose.
-__global__ void k_chol_stage(const double* gram, int R, int stage, int last, double shift, double out_scale,
-                             double s_scale, int transS, double* apply, double* Rtot, double* Sout, int* status) {
-    __shared__ double G[DLR_RMAXS][DLR_RMAXS + 1], U[DLR_RMAXS][DLR_RMAXS + 1], Ui[DLR_RMAXS][DLR_RMAXS + 1];
-    __shared__ double dsc[DLR_RMAXS], Rn[DLR_RMAXS][DLR_RMAXS + 1];
-    const int lane = threadIdx.x;
-    const int P = R * (R + 1) / 2;
-    if (lane < R) {
-        const int l = lane;
-        for (int a = 0; a < R; a++) {
-            const int lo = min(a, l), hi = max(a, l);
-            G[a][l] = sum_g1(gram, P, lo * R - lo * (lo - 1) / 2 + (hi - lo));
-            U[a][l] = 0.0; Ui[a][l] = 0.0;
-        }
-    }
-    __syncwarp();
-    if (lane < R) {
-        const double g = G[lane][lane];
-        dsc[lane] = g > 0.0 ? 1.0 / sqrt(g) : 1.0;
-    }
-    __syncwarp();
-    if (lane < R)
-        for (int a = 0; a < R; a++) {
-            G[a][lane] *= dsc[a] * dsc[lane];
-            if (a == lane && stage == 0) G[a][lane] += shift;
-        }
-    __syncwarp();
-    // upper Cholesky G = U^T U, lane = column
-    for (int j = 0; j < R; j++) {
-        if (lane == j) {
-            double s = G[j][j];
-            for (int k = 0; k < j; k++) s -= U[k][j] * U[k][j];
-            if (!(s > 1e-30)) { s = 1e-30; atomicAdd(status, 1); }     // repaired pivot (counted as a QR fallback)
-            U[j][j] = sqrt(s);
-        }
-        __syncwarp();
-        if (lane > j && lane < R) {
-            double s = G[j][lane];
-            for (int k = 0; k < j; k++) s -= U[k][j] * U[k][lane];
-            U[j][lane] = s / U[j][j];
-        }
-        __syncwarp();
-    }
-    // inverse of U (upper), lane = column l: U x = e_l
-    if (lane < R) {
-        const int l = lane;
-        Ui[l][l] = 1.0 / U[l][l];
-        for (int i = l - 1; i >= 0; i--) {
-            double s = 0.0;
-            for (int k = i + 1; k <= l; k++) s += U[i][k] * Ui[k][l];
-            Ui[i][l] = -s / U[i][i];
-        }
-    }
-    __syncwarp();
-    if (lane < R) {
-        const int l = lane;
-        const double osc = last ? out_scale : 1.0;
-        for (int a = 0; a < R; a++) apply[a * R + l] = dsc[a] * Ui[a][l] * osc;
-        // R_stage = U D^-1 ;  Rtot <- R_stage * Rtot
-        for (int a = 0; a < R; a++) {
-            double s = 0.0;
-            if (stage == 0) s = U[a][l] / dsc[l];
-            else
-                for (int k = a; k <= l; k++) s += (U[a][k] / dsc[k]) * Rtot[k * R + l];
-            Rn[a][l] = (a <= l) ? s : 0.0;
-        }
-    }
-    __syncwarp();
-    if (lane < R) {
-        const int l = lane;
-        for (int a = 0; a < R; a++) {
-            Rtot[a * R + l] = Rn[a][l];
-            if (last) {
-                if (transS) Sout[l + R * a] = Rn[a][l] * s_scale;      // S = R^T
-                else Sout[a + R * l] = Rn[a][l] * s_scale;             // S = R
+// The r x r work between two streaming phases in ONE launch (single CTA), each part optional:
+//   do_m2 : derivative coefficients M2_i = h^3 A^T d_i A (antisymmetric) from the Parseval partial
+//           sums of the dimension-3 pass: pgram [nblocks][3 P2], entry (a<b) of direction d at d*P2 + pe2;
+//   do_s  : S step, one RK4 step of eq. (10);
+//   do_tab: tables of the next K- or L-flow (mode-mixing matrices, phases, phi functions).
+struct PostArgs {
+    int R, do_m2, do_s, do_tab;
+    const double* pgram; int nblocks; double m2scale; double* M2;
+    double* S; double ts; const double *C1, *C2, *D1, *D2;
+    const double *Tm, *lam, *Sin; int transS; GridDev g; double sgn, tsub, t3; const double* M2c; double nlsign;
+    FlowTabPtrs o;
+};
+
+__global__ void __launch_bounds__(DLR_SMALL_THREADS) k_post(const PostArgs a) {
+    __shared__ SflowScratch sc;
+    __shared__ double red[DLR_RMAXS * (DLR_RMAXS - 1) / 2], tmp[DLR_SMALL_THREADS];
+    const int R = a.R, RR = R * R;
+    if (a.do_m2) {
+        const int P2 = R * (R - 1) / 2;
+        for (int d = 0; d < 3; d++) {
+            cta_reduce_rows(a.pgram, a.nblocks, 3 * P2, d * P2, P2, red, tmp);
+            for (int idx = threadIdx.x; idx < RR; idx += blockDim.x) {
+                const int i = idx / R, j = idx - i * R;
+                double v = 0.0;
+                if (i != j) {
+                    const int lo = min(i, j), hi = max(i, j);
+                    v = a.m2scale * red[lo * (R - 1) - lo * (lo - 1) / 2 + (hi - lo - 1)];
+                    if (i > j) v = -v;
+                }
+                a.M2[(size_t)d * RR + idx] = v;
             }
+            __syncthreads();
         }
+        __threadfence_block();
+        __syncthreads();
     }
+    if (a.do_s) {
+        dev_sflow(a.S, R, a.ts, a.C1, a.C2, a.D1, a.D2, sc);
+        __threadfence_block();
+        __syncthreads();
+    }
+    if (a.do_tab) dev_flow_tables(a.Tm, a.lam, a.Sin, a.transS, R, a.g, a.sgn, a.tsub, a.t3, a.M2c, a.nlsign, a.o);
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// vectors for the charge density: out[c] = scale * sum_j S(c,j) vec[j]   (use_S) or scale * vec[c]
-__global__ void k_rho_vec(const double* S, const double* vec, int R, int use_S, double scale, double* out) {
-    const int c = threadIdx.x;
-    if (c >= R) return;
-    double s = 0.0;
-    if (use_S == 2) for (int j = 0; j < R; j++) s += S[c + R * j] * vec[5 * j];      // vec = column moments, stride 5
-    else if (use_S) for (int j = 0; j < R; j++) s += S[c + R * j] * vec[j];
-    else s = vec[c];
-    out[c] = scale * s;
+// One stage of (shifted) CholeskyQR (single CTA): reduces the Gram partial sums of the producing pass itself, then
+// works entirely in shared memory (right-looking Cholesky over the whole CTA; no global loads or divisions inside
+// dependent loops).
+//   partial: [nblocks][P] upper pairs of A^T A.   stage 0 adds `shift` to the unit-diagonal scaled Gram matrix.
+//   apply[ci][co] : matrix for the next A*Mat pass (= D U^-1, times out_scale on the last stage)
+//   Rtot (row-major, upper triangular) accumulates R_stage * Rtot with R_stage = U D^-1.
+//   On the last stage the coupling matrix is written: Sout column-major = Rtot*s_scale (transS=0) or its transpose.
+__global__ void __launch_bounds__(DLR_SMALL_THREADS)
+k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, double shift, double out_scale,
+             double s_scale, int transS, double* apply, double* Rtot, double* Sout, int* status) {
+    __shared__ double G[DLR_RMAXS][DLR_RMAXS + 1], U[DLR_RMAXS][DLR_RMAXS + 1], Ui[DLR_RMAXS][DLR_RMAXS + 1];
+    __shared__ double Rp[DLR_RMAXS][DLR_RMAXS + 1];
+    __shared__ double dsc[DLR_RMAXS], sg[DLR_RMAXS], dinv[DLR_RMAXS];
+    __shared__ double red[DLR_RMAXS * (DLR_RMAXS + 1) / 2], tmp[DLR_SMALL_THREADS];
+    const int tid = threadIdx.x, nth = blockDim.x;
+    const int P = R * (R + 1) / 2, RR = R * R;
+    for (int idx = tid; idx < RR; idx += nth) {                 // previous Rtot (identity before the first stage)
+        const int i = idx / R, j = idx - i * R;
+        Rp[i][j] = stage ? Rtot[idx] : (i == j ? 1.0 : 0.0);
+    }
+    cta_reduce_rows(partial, nblocks, P, 0, P, red, tmp);
+    if (tid < R) {
+        const double g = red[tid * R - tid * (tid - 1) / 2];
+        dsc[tid] = g > 0.0 ? 1.0 / sqrt(g) : 1.0;
+        sg[tid] = g > 0.0 ? sqrt(g) : 1.0;
+    }
+    __syncthreads();
+    for (int idx = tid; idx < RR; idx += nth) {
+        const int i = idx / R, j = idx - i * R;
+        const int lo = min(i, j), hi = max(i, j);
+        double g = red[lo * R - lo * (lo - 1) / 2 + (hi - lo)] * dsc[i] * dsc[j];
+        if (i == j && stage == 0) g += shift;
+        G[i][j] = g;
+        U[i][j] = 0.0;
+        Ui[i][j] = 0.0;
+    }
+    __syncthreads();
+    // right-looking upper Cholesky G = U^T U
+    for (int j = 0; j < R; j++) {
+        if (tid == 0) {
+            double sjj = G[j][j];
+            if (!(sjj > 1e-30)) { sjj = 1e-30; atomicAdd(status, 1); }     // repaired pivot (counted as a QR fallback)
+            const double dj = sqrt(sjj);
+            U[j][j] = dj;
+            dinv[j] = 1.0 / dj;
+        }
+        __syncthreads();
+        if (tid > j && tid < R) U[j][tid] = G[j][tid] * dinv[j];
+        __syncthreads();
+        for (int idx = tid; idx < RR; idx += nth) {
+            const int i = idx / R, l = idx - i * R;
+            if (i > j && l >= i) G[i][l] -= U[j][i] * U[j][l];
+        }
+        __syncthreads();
+    }
+    // inverse of U (upper triangular), thread l = column l: back substitution
+    if (tid < R) {
+        const int l = tid;
+        Ui[l][l] = dinv[l];
+        for (int i = l - 1; i >= 0; i--) {
+            double sacc = 0.0;
+            for (int k = i + 1; k <= l; k++) sacc = fma(U[i][k], Ui[k][l], sacc);
+            Ui[i][l] = -sacc * dinv[i];
+        }
+    }
+    __syncthreads();
+    const double osc = last ? out_scale : 1.0;
+    for (int idx = tid; idx < RR; idx += nth) {
+        const int a = idx / R, l = idx - a * R;
+        apply[idx] = dsc[a] * Ui[a][l] * osc;
+        double sacc = 0.0;                                      // (U D^-1 Rp)[a][l], upper triangular
+        if (a <= l)
+            for (int k = a; k <= l; k++) sacc = fma(U[a][k] * sg[k], Rp[k][l], sacc);
+        Rtot[idx] = sacc;
+        if (last) {
+            if (transS) Sout[l + R * a] = sacc * s_scale;       // S = R^T
+            else Sout[a + R * l] = sacc * s_scale;              // S = R
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // diagnostics
-// column sums with weights {1, w1, w2, w3, |w|^2} (w = grid coordinate): out[c*5+m]; one CTA per column
-__global__ void k_colmoments(const double* A, GridDev g, double* out) {
-    __shared__ double red[5][32];
-    const int c = blockIdx.x, n = g.n;
+// column sums with weights {1, w1, w2, w3, |w|^2} (w = grid coordinate), two levels, fixed order:
+//   k_colmoments: grid (R, DLR_MCH); CTA (c, ch) sums a contiguous range of rows (lines along i1) of column c,
+//   one warp per row -> part[(c*DLR_MCH + ch)*5 + m];   k_colmoments_sum adds the DLR_MCH chunks -> out[c*5 + m].
+#define DLR_MCH 32
+__global__ void __launch_bounds__(256) k_colmoments(const double* A, GridDev g, double* part) {
+    __shared__ double red[5][8];
+    const int c = blockIdx.x, ch = blockIdx.y, n = g.n, lg = g.log2n;
+    const int rows = n << lg;                                   // n^2 rows of n points
+    const int per = (rows + DLR_MCH - 1) / DLR_MCH;
+    const int r0 = ch * per, r1 = min(rows, r0 + per);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const double* col = A + (size_t)c * g.N;
     double s[5] = {0, 0, 0, 0, 0};
-    for (long long I = threadIdx.x; I < g.N; I += blockDim.x) {
-        const int i1 = (int)(I % n), i2 = (int)((I / n) % n), i3 = (int)(I / ((long long)n * n));
-        const double w1 = g.lo + g.h * i1, w2 = g.lo + g.h * i2, w3 = g.lo + g.h * i3, a = col[I];
-        s[0] += a; s[1] += a * w1; s[2] += a * w2; s[3] += a * w3; s[4] += a * (w1 * w1 + w2 * w2 + w3 * w3);
+    for (int q = r0 + w; q < r1; q += nw) {
+        const int i2 = q & (n - 1), i3 = q >> lg;
+        const double w2 = g.lo + g.h * i2, w3 = g.lo + g.h * i3, w23 = w2 * w2 + w3 * w3;
+        const double* row = col + ((size_t)q << lg);
+        double t0 = 0.0, t1 = 0.0, t4 = 0.0;
+        for (int i1 = lane; i1 < n; i1 += 32) {
+            const double w1 = g.lo + g.h * i1, a = row[i1];
+            t0 += a; t1 += a * w1; t4 += a * (w1 * w1);
+        }
+        s[0] += t0; s[1] += t1; s[2] += t0 * w2; s[3] += t0 * w3; s[4] += t4 + t0 * w23;
     }
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (int m = 0; m < 5; m++) { s[m] = warp_sum(s[m]); if (lane == 0) red[m][w] = s[m]; }
     __syncthreads();
     if (threadIdx.x < 5) {
         double t = 0.0;
-        for (int i = 0; i < (int)(blockDim.x >> 5); i++) t += red[threadIdx.x][i];
-        out[c * 5 + threadIdx.x] = t;
+        for (int i = 0; i < nw; i++) t += red[threadIdx.x][i];
+        part[((size_t)c * DLR_MCH + ch) * 5 + threadIdx.x] = t;
     }
 }
 
-// sum of squares of nvals doubles -> out[0] (single CTA, fixed order)
-__global__ void k_sumsq(const double* a, long long nvals, double* out) {
-    __shared__ double red[32];
+__global__ void k_colmoments_sum(const double* partx, const double* partv, int R, double* mx, double* mv) {
+    for (int idx = threadIdx.x; idx < 2 * R * 5; idx += blockDim.x) {
+        const int which = idx / (R * 5), e = idx - which * R * 5, c = e / 5, m = e - c * 5;
+        const double* p = (which ? partv : partx) + (size_t)c * DLR_MCH * 5 + m;
+        double t = 0.0;
+        for (int ch = 0; ch < DLR_MCH; ch++) t += p[ch * 5];
+        (which ? mv : mx)[e] = t;
+    }
+}
+
+// partial sums of squares of nvals doubles -> out[blockIdx.x] (fixed order; k_moments_final adds the DLR_ECH parts)
+#define DLR_ECH 64
+__global__ void __launch_bounds__(256) k_sumsq(const double* a, long long nvals, double* out) {
+    __shared__ double red[8];
+    const long long per = (nvals + gridDim.x - 1) / gridDim.x;
+    const long long i0 = (long long)blockIdx.x * per, i1 = min(nvals, i0 + per);
     double s = 0.0;
-    for (long long i = threadIdx.x; i < nvals; i += blockDim.x) s = fma(a[i], a[i], s);
+    for (long long i = i0 + threadIdx.x; i < i1; i += blockDim.x) s = fma(a[i], a[i], s);
     s = warp_sum(s);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
     __syncthreads();
     if (threadIdx.x == 0) {
         double t = 0.0;
         for (int i = 0; i < (int)(blockDim.x >> 5); i++) t += red[i];
-        out[0] = t;
+        out[blockIdx.x] = t;
     }
 }
 
-// moments from the column moments; res: mass, mom1..3, kinetic, s_fro, nonfinite
+// moments from the column moments; res: mass, mom1..3, kinetic, s_fro, nonfinite, sum |E|^2
 __global__ void k_moments_final(const double* mx, const double* mv, const double* S, int R, double hx3, double hv3,
-                                double* res) {
+                                const double* epart, double* res) {
     if (threadIdx.x != 0) return;
     double out[5] = {0, 0, 0, 0, 0}, fro = 0.0;
     int bad = 0;
@@ -398,8 +505,10 @@ __global__ void k_moments_final(const double* mx, const double* mv, const double
             fro += s * s;
             for (int m = 0; m < 5; m++) out[m] += hx3 * mx[i * 5] * s * hv3 * mv[j * 5 + m];
         }
+    double es = 0.0;
+    for (int i = 0; i < DLR_ECH; i++) es += epart[i];
     res[0] = out[0]; res[1] = out[1]; res[2] = out[2]; res[3] = out[3]; res[4] = 0.5 * out[4];
-    res[5] = sqrt(fro); res[6] = (double)bad;
+    res[5] = sqrt(fro); res[6] = (double)bad; res[7] = es;
 }
 
 __global__ void k_probes(const double* X, const double* S, const double* V, long long Nx, long long Nv, int R, int np,

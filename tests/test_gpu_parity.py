@@ -27,6 +27,16 @@ def rel(a, b):
     return abs(a - b) / abs(b)
 
 
+def ee_scale(hist, m):
+    """normalisation of the electric-energy error at step m of a history (reading R17): the value itself,
+    except at a strict local minimum of the oracle's history, where the field passes (almost) through zero and the
+    pointwise relative error of 1/2 |E|^2 is ill-conditioned (fp64 rounding floor ~1e-13 * ee(0) divided by a value
+    1e-5 * ee(0)); there the larger of the two neighbouring samples is used."""
+    if 0 < m < len(hist) - 1 and hist[m] < hist[m - 1] and hist[m] < hist[m + 1]:
+        return max(hist[m - 1], hist[m + 1])
+    return hist[m]
+
+
 def make_ctx(cfg, order=2, e_scale=1.0):
     from paper_2110_13481_b200 import dlr
     return dlr.Dlr(dlr.config_from_inputs(cfg, order=order, e_scale=e_scale))
@@ -117,11 +127,14 @@ def test_full_run_config1():
     ix, iv = inputs.probe_indices(cfg)
     ctx = make_ctx(cfg)
     ctx.set_initial(X, S, V)
+    ee_gpu, ee_ora = [ctx.moments()["electric_energy"]], [O.moments(X, S, V, gx, gv)["electric_energy"]]
     for _ in range(cfg["steps"]):
         ctx.step(cfg["tau"])
         X, S, V = O.step_alg2(X, S, V, cfg["tau"], gx, gv)
-        m = ctx.moments()
-        assert rel(m["electric_energy"], O.moments(X, S, V, gx, gv)["electric_energy"]) <= TOL_RUN
+        ee_gpu.append(ctx.moments()["electric_energy"])
+        ee_ora.append(O.moments(X, S, V, gx, gv)["electric_energy"])
+    for m in range(len(ee_ora)):
+        assert abs(ee_gpu[m] - ee_ora[m]) <= (TOL_STEP if m <= 1 else TOL_RUN) * ee_scale(ee_ora, m), m
     check(ctx, X, S, V, gx, gv, ix, iv, TOL_RUN)
     ctx.close()
 
@@ -148,7 +161,8 @@ def _golden_run(idx, max_steps=None):
             assert np.abs(f - fo).max() <= tol * np.abs(fo).max(), step
         else:
             m = ctx.moments()
-        assert rel(m["electric_energy"], gold["electric_energy"][step]) <= tol, step
+        ee = gold["electric_energy"]
+        assert abs(m["electric_energy"] - ee[step]) <= tol * ee_scale(ee[:nsteps + 1], step), step
         assert rel(m["mass"], gold["mass"][step]) <= tol, step
         assert rel(m["kinetic_energy"], gold["kinetic_energy"][step]) <= tol, step
         assert m["qr_fallbacks"] == 0 and m["nonfinite"] == 0
