@@ -110,9 +110,11 @@ int dlr_launches_per_step(dlr_ctx* ctx);
 /* Algorithmic bytes one dlr_step moves under the byte model of DESIGN.md section 6 (for the roofline). */
 double dlr_bytes_per_step(dlr_ctx* ctx);
 
-/* Kernel-level entry points for tests and micro-benchmarks (all pointers DEVICE, stream of ctx):
- * batched 3D real-to-complex FFT of ncols columns on the x grid (which = 0) or v grid (which = 1) into the
- * library's internal half-spectrum layout, and back (out = in up to rounding).  ncols must be the rank, 1 or 3. */
+/* Kernel-level entry point for tests (all pointers DEVICE, stream of ctx): the batched 3D real-to-complex FFT of
+ * the Poisson solve on ncols = 3 columns of the x grid (which = 0; which = 1: the v grid, only if
+ * it is not larger than the x grid) into the library's half-spectrum layout (k1 natural 0..n/2, k2 and k3 at
+ * bit-reversed positions), and back (out = in up to rounding).  Other ncols: DLR_ERR_UNSUPPORTED.  The K/L flows
+ * themselves use 1D transforms inside their passes and are tested through dlr_step. */
 int dlr_test_fft_roundtrip(dlr_ctx* ctx, int which, int ncols, const double* d_in, double* d_out,
                            double* d_spec /* 2*ncols*(n/2+1)*n*n doubles */);
 

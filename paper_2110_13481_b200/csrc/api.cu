@@ -41,6 +41,8 @@ struct HostGrid {
     int T3, T3s;          // pencils per CTA in dimension-3 passes
     int T2, NB2, nch2;    // dimension-2 pass tiling
     int thr1, thr2, thr3; // CTA sizes of the three pass families
+    int Lx, Le, Lc;       // directional passes: packed lines per column for EXACT, ETD and COEFF tiles
+    int thrd;             // CTA size of the directional passes
 };
 
 struct FlowTab {
@@ -63,10 +65,10 @@ struct dlr_ctx {
     const RankOps* ops;
     HostGrid gx, gv;
     // big buffers
-    double *X, *V, *S, *Sp;
-    double2 *Xh0, *Xh, *Vh, *W, *MB, *Eh;
-    double *KL, *Q1, *E;
-    double *partial, *partialP, *partial2a;
+    double *X, *X1, *V, *S, *Sp;     // X1: the predictor basis of Algorithm 2 (X itself stays X0 until the first K step)
+    double2* Eh;
+    double *KL, *Q1, *W, *E;
+    double *partial, *partialP[3], *partialC, *partial2a;
     // small buffers
     double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *zsum, *mx, *mv, *mxp, *mvp, *mres, *esum;
     int* status;
@@ -150,6 +152,14 @@ void choose_T2(int n, int nh, int& T2, int& NB, int& nch) {
     while (NB > 1 && d2_smem_bytes(n, T2, NB) > SMEM_MAX) NB--;
 }
 
+// packed lines per column of a directional tile: the largest power of two <= lmax whose tile fits the target
+int choose_L(int n, int R, int nbuf, int nmat, bool needE, size_t target, int lmax) {
+    int best = 1;
+    for (int L = 1; L <= lmax && L <= n / 2; L *= 2)
+        if (dir_smem_bytes(n, R, L, nbuf, nmat, needE) <= target) best = L;
+    return best;
+}
+
 struct Carver {
     char* base;
     size_t off;
@@ -184,18 +194,15 @@ size_t grid_table_doubles(int n) { return (size_t)(2 * (n / 2 + 1) + 2 * n + n) 
 // carve the workspace; with base == nullptr only measures
 size_t carve(dlr_ctx* c, char* base) {
     const int R = c->R;
-    const long long Nx = c->gx.g.N, Nv = c->gv.g.N, NCx = c->gx.g.NC, NCv = c->gv.g.NC;
-    const long long Nmax = Nx > Nv ? Nx : Nv, NCmax = NCx > NCv ? NCx : NCv;
+    const long long Nx = c->gx.g.N, Nv = c->gv.g.N, NCx = c->gx.g.NC;
+    const long long Nmax = Nx > Nv ? Nx : Nv;
     Carver cv{base, 0};
     c->X = cv.take<double>((size_t)Nx * R);
+    c->X1 = cv.take<double>((size_t)Nx * R);
     c->V = cv.take<double>((size_t)Nv * R);
     c->KL = cv.take<double>((size_t)Nmax * R);
     c->Q1 = cv.take<double>((size_t)Nmax * R);
-    c->Xh0 = cv.take<double2>((size_t)NCx * R);
-    c->Xh = cv.take<double2>((size_t)NCx * R);
-    c->Vh = cv.take<double2>((size_t)NCv * R);
-    c->W = cv.take<double2>((size_t)NCmax * R);
-    c->MB = cv.take<double2>((size_t)NCmax * R);
+    c->W = cv.take<double>((size_t)Nmax * R);
     c->E = cv.take<double>((size_t)3 * Nx);
     c->Eh = cv.take<double2>((size_t)3 * NCx);
     // per-CTA partial sums: the largest producer is a dimension-1 pass with the weighted Gram
@@ -203,12 +210,14 @@ size_t carve(dlr_ctx* c, char* base) {
     size_t blocks = 0;
     for (const HostGrid* hg : {&c->gx, &c->gv}) {
         size_t b1 = (size_t)hg->g.n * hg->g.n / hg->T1;
-        size_t b3 = ((size_t)hg->g.nh * hg->g.n + hg->T3 - 1) / hg->T3;
-        blocks = std::max(blocks, std::max(b1, b3));
+        size_t bd = (size_t)dir_tiles(hg->g.n, 1);            // directional tiles at L = 1 (the most there can be)
+        bd = std::max(bd / hg->Lx, std::max(bd / hg->Le, bd / hg->Lc));
+        blocks = std::max(blocks, std::max(b1, bd));
     }
     c->partial_cap = blocks * nvmax;
     c->partial = cv.take<double>(c->partial_cap);
-    c->partialP = cv.take<double>(blocks * (size_t)(3 * R * (R - 1) / 2));   // Parseval sums of the dimension-3 pass
+    for (int d = 0; d < 3; d++) c->partialP[d] = cv.take<double>(blocks * (size_t)(R * (R - 1) / 2));   // Parseval sums
+    c->partialC = cv.take<double>(blocks * (size_t)R);                                                  // column sums
     c->partial2a = cv.take<double>((size_t)DLR_G1 * nvmax);
     const int RR = R * R;
     c->S = cv.take<double>(RR); c->Sp = cv.take<double>(RR);
@@ -224,10 +233,10 @@ size_t carve(dlr_ctx* c, char* base) {
     c->status = cv.take<int>(4);
     c->probe_cap = 4096;
     c->pix = cv.take<long long>(c->probe_cap); c->piv = cv.take<long long>(c->probe_cap); c->pf = cv.take<double>(c->probe_cap);
-    const int nmax = std::max(c->gx.g.n, c->gv.g.n), nhmax = nmax / 2 + 1;
+    const int nmax = std::max(c->gx.g.n, c->gv.g.n);
     c->ft.p.mats = cv.take<double>(8 * RR);
-    c->ft.p.nl = cv.take<double>(3 * RR);
-    c->ft.p.ph1 = cv.take<double2>((size_t)nhmax * R);
+    c->ft.p.Q = cv.take<double>(3 * RR);
+    c->ft.p.ph1 = cv.take<double2>((size_t)nmax * R);
     c->ft.p.ph2 = cv.take<double2>((size_t)nmax * R);
     c->ft.p.ez = cv.take<double2>((size_t)nmax * R);
     c->ft.p.f1 = cv.take<double2>((size_t)nmax * R);
@@ -260,6 +269,15 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     hg.thr1 = valid_threads(tune("thr1", DLR_THREADS));
     hg.thr2 = valid_threads(tune("thr2", DLR_THREADS));
     hg.thr3 = valid_threads(tune("thr3", DLR_THREADS));
+    hg.thrd = valid_threads(tune("thrd", DLR_THREADS));
+    const int lmax = 8;
+    hg.Lx = choose_L(n, R, 1, 2, false, (size_t)tune("smx", 48) * 1024, lmax);
+    hg.Le = choose_L(n, R, 2, 5, true, (size_t)tune("sme", 110) * 1024, lmax);
+    hg.Lc = choose_L(n, R, 1, 2, true, (size_t)tune("smc", 64) * 1024, lmax);
+    const int lx = tune("lx", 0), le = tune("le", 0), lc = tune("lc", 0);
+    if (is_pow2(lx) && lx <= n / 2 && dir_smem_bytes(n, R, lx, 1, 2, false) <= SMEM_MAX) hg.Lx = lx;
+    if (is_pow2(le) && le <= n / 2 && dir_smem_bytes(n, R, le, 2, 5, true) <= SMEM_MAX) hg.Le = le;
+    if (is_pow2(lc) && lc <= n / 2 && dir_smem_bytes(n, R, lc, 1, 2, true) <= SMEM_MAX) hg.Lc = lc;
 }
 
 cudaError_t upload_tables(dlr_ctx* c, HostGrid& hg, double lo, double hi) {
@@ -329,7 +347,6 @@ D3Args d3args(dlr_ctx* c, const HostGrid& hg) {
     memset(&a, 0, sizeof(a));
     a.g = hg.g; a.T = hg.T3; a.e_scale = c->cfg.e_scale; a.threads = hg.thr3;
     a.mats = c->ft.p.mats; a.ph1 = c->ft.p.ph1; a.ph2 = c->ft.p.ph2; a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1;
-    a.mbuf = c->MB;
     return a;
 }
 
@@ -341,34 +358,38 @@ void reduce_partials(dlr_ctx* c, int nblocks, int nvals, double* out2) {
 int d1_blocks(const HostGrid& hg) { return (int)((long long)hg.g.n * hg.g.n / hg.T1); }
 int d3_blocks(const HostGrid& hg) { return (int)(((long long)hg.g.nh * hg.g.n + hg.T3 - 1) / hg.T3); }
 
-// Factor transform: A (real, N x r) -> Ah (half spectrum), accumulating the coefficient sums on the way:
-// kind = 0: none;  1: C coefficients (weights v_i, + rho_tilde);  2: D coefficients (weights E_i).
-// With kind != 0: M1 (C1 or D1), its eigen-decomposition (T, lam) and colsum are final when this returns (in stream
-// order); the Parseval sums of the derivative coefficients are left in c->partialP for post(..., do_m2).
-void factor_fft(dlr_ctx* c, const HostGrid& hg, const double* A, double2* Ah, int kind, double* M1, double* colsum,
-                double* T, double* lam) {
+DirArgs dirargs(const HostGrid& hg) {
+    DirArgs a;
+    memset(&a, 0, sizeof(a));
+    a.g = hg.g; a.threads = hg.thrd;
+    return a;
+}
+int dir_blocks(const HostGrid& hg, int L) { return dir_tiles(hg.g.n, L); }
+
+// Coefficient set of a factor A (N x r, real):  kind = 1: C coefficients (weights v_i, + rho_tilde);  2: D coefficients
+// (weights E_i).  Three read-only passes, one per direction: the first also accumulates the real-space weighted Gram
+// (M1 = C1 or D1, colsum), each leaves the 1D Parseval sums of its derivative coefficient in c->partialP[d] for
+// post(..., do_m2).  M1, its eigen-decomposition (T, lam) and colsum are final when this returns (in stream order).
+void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M1, double* colsum, double* T, double* lam) {
     const int R = c->R;
-    D1Args a = d1args(hg);
-    a.in_real = A; a.out_cplx = Ah; a.E = c->E; a.partial = c->partial;
-    CK(c->ops->d1[kind == 0 ? V1_FFT_PLAIN : kind == 1 ? V1_FFT_GRAMV : V1_FFT_GRAME](a, c->st));
-    if (kind) {
-        // fork: M1 and its eigen-decomposition need only the Gram sums of the pass above; they run beside the two
-        // remaining passes of the transform (under stream capture this becomes a parallel branch of the step graph)
-        CK(cudaEventRecord(c->ev_fork, c->st));
-        CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-        k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->partial, d1_blocks(hg), R, kind == 1, hg.g.h3, M1, colsum, T, lam);
-        CK(cudaGetLastError());
-        CK(cudaEventRecord(c->ev_join, c->side));
-        c->count_launches -= 3;                     // the three event calls above are not kernel launches
-    }
-    run_d2(c, hg, Ah, R, false);
-    D3Args b = d3args(c, hg);
-    b.in = Ah; b.out = Ah; b.partial = c->partialP;
-    CK(c->ops->d3[kind ? V3_FWD_PGRAM : V3_FWD](b, c->st));
-    if (kind) {
-        CK(cudaStreamWaitEvent(c->st, c->ev_join, 0));      // join before anything reads M1, T, lam, colsum
-        c->count_launches -= 1;
-    }
+    DirArgs a = dirargs(hg);
+    a.in = A; a.E = c->E; a.L = hg.Lc; a.gram = c->partial; a.pgram = c->partialP[0];
+    CK(c->ops->dir[kind == 1 ? VD_COEFF1_V : VD_COEFF1_E](a, c->st));
+    // fork: M1 and its eigen-decomposition need only the Gram sums of the pass above; they run beside the two
+    // remaining passes (under stream capture this becomes a parallel branch of the step graph)
+    CK(cudaEventRecord(c->ev_fork, c->st));
+    CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->partial, dir_blocks(hg, hg.Lc), R, kind == 1, hg.g.h3, M1, colsum, T, lam);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(c->ev_join, c->side));
+    c->count_launches -= 3;                         // the three event calls above are not kernel launches
+    a.gram = nullptr; a.E = nullptr;
+    a.pgram = c->partialP[1];
+    CK(c->ops->dir[VD_COEFF2](a, c->st));
+    a.pgram = c->partialP[2];
+    CK(c->ops->dir[VD_COEFF3](a, c->st));
+    CK(cudaStreamWaitEvent(c->st, c->ev_join, 0));  // join before anything reads M1, T, lam, colsum
+    c->count_launches -= 1;
 }
 
 // The r x r work between two streaming phases, one launch (see k_post).
@@ -380,8 +401,9 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
     memset(&a, 0, sizeof(a));
     a.R = c->R;
     if (m2) {
-        a.do_m2 = 1; a.pgram = c->partialP; a.nblocks = d3_blocks(*m2->hg);
-        a.m2scale = m2->hg->g.h3 / (double)m2->hg->g.N; a.M2 = m2->M2;
+        a.do_m2 = 1; a.nblocks = dir_blocks(*m2->hg, m2->hg->Lc);
+        for (int d = 0; d < 3; d++) a.pgram[d] = c->partialP[d];
+        a.m2scale = m2->hg->g.h3 / (double)m2->hg->g.n; a.M2 = m2->M2;     // 1D Parseval: sum_x u dv = (1/n) sum_k ...
     }
     if (sf) { a.do_s = 1; a.S = sf->S; a.ts = sf->t; a.C1 = c->C1; a.C2 = c->C2; a.D1 = c->D1; a.D2 = c->D2; }
     if (tb) {
@@ -412,15 +434,17 @@ void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int 
 
 // shifted CholeskyQR3 of KL (N x r) -> orthonormal basis (h^3 B^T B = I) into `basis`, coupling matrix into Sout
 // (transS: S = R^T for the L step, Fig. 1 line 40 transpose_inplace).
-// The Gram sums of KL must already be in c->partial (written by the pass that produced KL).
-void qr(dlr_ctx* c, const HostGrid& hg, double* basis, double* Sout, int transS) {
+// The Gram sums of KL must already be in c->partial, one row per CTA of the pass that produced KL (nblocks0 rows).
+void qr(dlr_ctx* c, const HostGrid& hg, int nblocks0, double* basis, double* Sout, int transS) {
     const int R = c->R;
     const double shift = 64.0 * R * 2.220446049250313e-16;
     const double osc = 1.0 / sqrt(hg.g.h3), ssc = sqrt(hg.g.h3);
     double* src[3] = {c->KL, c->Q1, c->KL};
     double* dst[3] = {c->Q1, c->KL, basis};
     for (int stage = 0; stage < 3; stage++) {
-        k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->partial, d1_blocks(hg), R, stage, stage == 2, shift, osc, ssc,
+        // stage 0 reads the Gram sums written by the last pass of the flow (nblocks0 tiles), later stages those of
+        // the previous A*Mat pass
+        k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->partial, stage == 0 ? nblocks0 : d1_blocks(hg), R, stage, stage == 2, shift, osc, ssc,
                                                           transS, c->apply, c->Rtot, Sout, c->status);
         CK(cudaGetLastError());
         D1Args a = d1args(hg);
@@ -429,40 +453,44 @@ void qr(dlr_ctx* c, const HostGrid& hg, double* basis, double* Sout, int transS)
     }
 }
 
-// K- or L-flow of section 4 starting from the spectrum `spec` of the basis (the product with the
-// coupling matrix is folded into the first mode-mixing matrix).  order 1: Lie + exponential Euler; order 2: Strang +
-// ETD2RK.  Result: real factor in c->KL with its Gram sums in c->partial, or (zero_only) only the column sums of
-// the result (without the h^3 weight) in c->zsum.
-void flow(dlr_ctx* c, const HostGrid& hg, const double2* spec, bool is_L, int order, bool zero_only) {
+// K- or L-flow of section 4 of the factor `src` (X or V; the product with the coupling matrix is
+// folded into the first column-mixing matrix).  order 1: Lie + exponential Euler = 3 directional passes;
+// order 2: Strang + ETD2RK = 5 passes (1, 2, 3, 2, 1).  Result: real factor in c->KL with its Gram sums in c->partial,
+// or (zero_only) only the column sums of the result (without the h^3 weight) in c->zsum.  Returns the number of
+// Gram partial rows written.
+int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order, bool zero_only) {
     const RankOps* ops = c->ops;
-    const int vmid = is_L ? V1_MID_V : V1_MID_E;
-    D3Args s = d3args(c, hg);
-    s.in = spec; s.out = c->W;
-    CK(ops->d3[V3_START](s, c->st));
-    run_d2(c, hg, c->W, c->R, true);
-    D1Args m = d1args(hg);
-    m.in_cplx = c->W; m.out_cplx = c->W; m.mat = c->ft.p.nl; m.E = c->E;
-    CK(ops->d1[vmid](m, c->st));
-    run_d2(c, hg, c->W, c->R, false);
-    D3Args e = d3args(c, hg);
-    e.in = c->W; e.out = c->W;
+    const int RR = c->R * c->R;
+    const double* mats = c->ft.p.mats;
+    DirArgs a = dirargs(hg);
+    a.store = 1; a.L = hg.Lx;
+    // sub-flow 1:  A <- src (Sin T1), phases, then into the eigenbasis of direction 2
+    a.in = src; a.out = c->W; a.min_ = mats + 0 * RR; a.mout = mats + 1 * RR; a.ph = c->ft.p.ph1;
+    CK(ops->dir[VD_EXACT1](a, c->st));
+    // sub-flow 2
+    a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
+    CK(ops->dir[VD_EXACT2](a, c->st));
+    // sub-flow 3 in the eigenbasis of direction 3
+    DirArgs e = dirargs(hg);
+    e.L = hg.Le; e.in = c->W; e.E = c->E; e.min_ = mats + 2 * RR; e.Q = c->ft.p.Q;
+    e.ez = c->ft.p.ez; e.f1 = c->ft.p.f1; e.f2a = c->ft.p.f2a; e.f2b = c->ft.p.f2b;
     if (order == 1) {
-        if (zero_only) { e.zero_out = c->zsum; e.skip_store = 1; }
-        CK(ops->d3[V3_EULER_END](e, c->st));
-        if (zero_only) return;
-    } else {
-        e.f2 = c->ft.p.f2a;
-        CK(ops->d3[V3_MID](e, c->st));
-        run_d2(c, hg, c->W, c->R, true);
-        CK(ops->d1[vmid](m, c->st));
-        run_d2(c, hg, c->W, c->R, false);
-        e.f2 = c->ft.p.f2b;
-        CK(ops->d3[V3_END2](e, c->st));
+        e.mout = mats + 3 * RR;                      // T3^T: back to the original basis
+        if (zero_only) { e.store = 0; e.colsum = c->partialC; }
+        else { e.store = 1; e.out = c->KL; e.gram = c->partial; }
+        CK(ops->dir[is_L ? VD_ETD1_V : VD_ETD1_E](e, c->st));
+        if (zero_only) {
+            k_colsum_reduce<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->partialC, dir_blocks(hg, hg.Le), c->R, c->zsum);
+            CK(cudaGetLastError());
+        }
+        return dir_blocks(hg, hg.Le);
     }
-    run_d2(c, hg, c->W, c->R, true);
-    D1Args o = d1args(hg);
-    o.in_cplx = c->W; o.out_real = c->KL; o.partial = c->partial;
-    CK(ops->d1[V1_INV_GRAM](o, c->st));
+    e.mout = mats + 5 * RR; e.store = 1; e.out = c->W;          // T3^T T2
+    CK(ops->dir[is_L ? VD_ETD2_V : VD_ETD2_E](e, c->st));
+    CK(ops->dir[VD_EXACT2](a, c->st));                           // sub-flow 2, second half
+    a.out = c->KL; a.min_ = mats + 6 * RR; a.mout = mats + 7 * RR; a.ph = c->ft.p.ph1; a.gram = c->partial;
+    CK(ops->dir[VD_EXACT1](a, c->st));                           // sub-flow 1, second half, + Gram of the result
+    return dir_blocks(hg, hg.Lx);
 }
 
 // one step, issued on c->st (directly or under stream capture)
@@ -475,12 +503,13 @@ void issue_step(dlr_ctx* c, double tau) {
     phase_mark(c, "start");
     // ---- Algorithm 1, line 1: C coefficients from V0 (kept from the previous step's line 10 when valid)
     if (!c->vh_valid) {
-        factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->rho_t, c->TC, c->lamC);
+        coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
         post(c, &m2C, nullptr, nullptr);
     }
     phase_mark(c, "C coefficients (V0)");
-    // ---- line 2: K0 = X0 S0, kept as the spectrum of X0 (the product with S0 is folded into the flow)
-    factor_fft(c, gx, c->X, c->Xh0, 0, nullptr, nullptr, nullptr, nullptr);
+    // ---- line 2: K0 = X0 S0 is never formed (the product with S0 is folded into the flow).  In Algorithm 2 the
+    //      predictor basis X1 goes to its own buffer: the corrector's first K step starts from X0 again.
+    double* Xp = order == 2 ? c->X1 : c->X;
     // ---- line 3: E0 from K0 and V0, eq. (12): rho = -X0 (S0 rho_tilde)
     field(c, c->X, c->S, c->rho_t, 1, -1.0);
     phase_mark(c, "electric field E0");
@@ -489,12 +518,12 @@ void issue_step(dlr_ctx* c, double tau) {
         const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, tp, tp, c->C2, 1.0};
         post(c, nullptr, nullptr, &tb);
     }
-    flow(c, gx, c->Xh0, false, 1, false);
+    int nb = flow(c, gx, c->X, false, 1, false);
     phase_mark(c, "K step (predictor)");
-    qr(c, gx, c->X, Sp, 0);
+    qr(c, gx, nb, Xp, Sp, 0);
     phase_mark(c, "QR K (predictor)");
     // ---- line 6: D coefficients from X1 and E0;  line 7: S step;  lines 8-9: L0 = V0 S2^T, tables of the L step
-    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, nullptr, c->TD, c->lamD);
+    coeffs(c, gx, Xp, 2, c->D1, nullptr, c->TD, c->lamD);
     phase_mark(c, "D coefficients (predictor)");
     {
         const PostS sf{Sp, tp};
@@ -503,29 +532,29 @@ void issue_step(dlr_ctx* c, double tau) {
     }
     phase_mark(c, "S step (predictor)");
     if (order == 1) {
-        flow(c, gv, c->Vh, true, 1, false);
+        nb = flow(c, gv, c->V, true, 1, false);
         phase_mark(c, "L step");
-        qr(c, gv, c->V, c->S, 1);                 // line 10: V1, S3 = R^T
+        qr(c, gv, nb, c->V, c->S, 1);                 // line 10: V1, S3 = R^T
         phase_mark(c, "QR L");
         c->vh_valid = false;
         return;
     }
-    flow(c, gv, c->Vh, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
+    flow(c, gv, c->V, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
     phase_mark(c, "L step (predictor)");
     // ---- Algorithm 2, line 2: E^{1/2} from X1 and L1, eq. (13)
-    field(c, c->X, nullptr, c->zsum, 1, -gv.g.h3);
+    field(c, Xp, nullptr, c->zsum, 1, -gv.g.h3);
     phase_mark(c, "electric field E1/2");
     // ---- line 3: K step (Strang, ETD2RK) of length tau/2 from K0 = X0 S0 with E^{1/2};  line 4: QR -> X2, S3
     {
         const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0};
         post(c, nullptr, nullptr, &tb);
     }
-    flow(c, gx, c->Xh0, false, 2, false);
+    nb = flow(c, gx, c->X, false, 2, false);
     phase_mark(c, "first K step");
-    qr(c, gx, c->X, c->S, 0);
+    qr(c, gx, nb, c->X, c->S, 0);
     phase_mark(c, "QR K (first)");
     // ---- line 5: D coefficients from X2 and E^{1/2};  line 6: S step;  tables of the L step (L = V0 S4^T)
-    factor_fft(c, gx, c->X, c->Xh, 2, c->D1, nullptr, c->TD, c->lamD);
+    coeffs(c, gx, c->X, 2, c->D1, nullptr, c->TD, c->lamD);
     phase_mark(c, "D coefficients");
     {
         const PostS sf{c->S, 0.5 * tau};
@@ -534,13 +563,13 @@ void issue_step(dlr_ctx* c, double tau) {
     }
     phase_mark(c, "first S step");
     // ---- lines 7-9: L step (Strang) of length tau, QR -> V1, S5 = R^T
-    flow(c, gv, c->Vh, true, 2, false);
+    nb = flow(c, gv, c->V, true, 2, false);
     phase_mark(c, "L step");
-    qr(c, gv, c->V, c->S, 1);
+    qr(c, gv, nb, c->V, c->S, 1);
     phase_mark(c, "QR L");
     // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step;
-    //      tables of the second K step (K3 = X2 S6; the spectrum of X2 is in Xh)
-    factor_fft(c, gv, c->V, c->Vh, 1, c->C1, c->rho_t, c->TC, c->lamC);
+    //      tables of the second K step (K3 = X2 S6)
+    coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
     phase_mark(c, "C coefficients");
     {
         const PostS sf{c->S, 0.5 * tau};
@@ -549,9 +578,9 @@ void issue_step(dlr_ctx* c, double tau) {
     }
     phase_mark(c, "second S step");
     // ---- lines 12-14: K step (Strang) of length tau/2, QR -> X3, S7
-    flow(c, gx, c->Xh, false, 2, false);
+    nb = flow(c, gx, c->X, false, 2, false);
     phase_mark(c, "second K step");
-    qr(c, gx, c->X, c->S, 0);
+    qr(c, gx, nb, c->X, c->S, 0);
     phase_mark(c, "QR K (second)");
     c->vh_valid = true;
 }
@@ -822,42 +851,29 @@ int dlr_get_field(dlr_ctx* c, double* E, int on_device) {
 
 int dlr_test_fft_roundtrip(dlr_ctx* c, int which, int ncols, const double* d_in, double* d_out, double* d_spec) {
     if (!c || !d_in || !d_out || !d_spec) return DLR_ERR_INVALID;
+    if (ncols != 3) return DLR_ERR_UNSUPPORTED;
     const HostGrid& hg = which ? c->gv : c->gx;
+    if (hg.g.NC > c->gx.g.NC) return DLR_ERR_UNSUPPORTED;      // the scratch spectrum is sized for the x grid
     double2* spec = (double2*)d_spec;
     D1Args a = d1args(hg);
-    a.in_real = d_in; a.out_cplx = spec;
+    a.in_real = d_in; a.out_cplx = spec; a.T = hg.T1s;
     D3Args b = d3args(c, hg);
-    b.in = spec; b.out = spec;
+    b.in = spec; b.out = spec; b.T = hg.T3s;
     D1Args e = d1args(hg);
-    e.in_cplx = spec; e.out_real = d_out;
-    if (ncols == c->R) {
-        CK(c->ops->d1[V1_FFT_PLAIN](a, c->st));
-        run_d2(c, hg, spec, ncols, false);
-        CK(c->ops->d3[V3_FWD](b, c->st));
-    } else if (ncols == 3) {
-        a.T = e.T = hg.T1s; b.T = hg.T3s;
-        CK((launch_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>(a, c->st)));
-        run_d2(c, hg, spec, ncols, false);
-        CK((launch_d3<3, 3, D3_FWD_STORE, false>(b, c->st)));
-    } else {
-        return DLR_ERR_UNSUPPORTED;
-    }
+    e.in_cplx = spec; e.out_real = d_out; e.T = hg.T1s;
+    CK((launch_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>(a, c->st)));
+    run_d2(c, hg, spec, ncols, false);
+    CK((launch_d3<3, 3, D3_FWD_STORE, false>(b, c->st)));
     cudaError_t er = cudaStreamSynchronize(c->st);
     if (er != cudaSuccess) return fail(c, er, "fft forward");
     // the inverse consumes a copy so that d_spec keeps the forward transform for inspection
-    double2* tmp = c->W;
+    double2* tmp = c->Eh;
     er = cudaMemcpyAsync(tmp, spec, (size_t)ncols * hg.g.NC * sizeof(double2), cudaMemcpyDeviceToDevice, c->st);
     if (er != cudaSuccess) return fail(c, er, "fft copy");
     b.in = tmp; b.out = tmp; e.in_cplx = tmp;
-    if (ncols == c->R) {
-        CK(c->ops->d3[V3_INV](b, c->st));
-        run_d2(c, hg, tmp, ncols, true);
-        CK(c->ops->d1[V1_INV](e, c->st));
-    } else {
-        CK((launch_d3<3, 3, D3_INV_ONLY, false>(b, c->st)));
-        run_d2(c, hg, tmp, ncols, true);
-        CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
-    }
+    CK((launch_d3<3, 3, D3_INV_ONLY, false>(b, c->st)));
+    run_d2(c, hg, tmp, ncols, true);
+    CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
     er = cudaStreamSynchronize(c->st);
     if (er != cudaSuccess) return fail(c, er, "fft inverse");
     return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;

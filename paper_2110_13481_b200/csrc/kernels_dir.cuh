@@ -1,0 +1,460 @@
+// Directional passes.  Every sub-flow of the K/L step involves the wavenumber of ONE direction only (eqs. (14)-(19),
+// PAPER.md:246-270 use the partial transforms F_{x_i}), so no 3D transform is ever formed: a pass loads a tile that
+// holds complete lines along its direction for ALL columns, transforms along that direction in shared memory, applies
+// the sub-flow, transforms back and stores REAL data - one read and one write of the factor per sub-flow.
+//
+//   DOP_EXACT : [A <- A*Min] -> FFT_d -> * exp(s i t k~_d lambda_j) -> IFFT_d -> [A <- A*Mout]      eqs. (14),(15),(17),(18)
+//   DOP_ETD1/2: third sub-flow in the eigenbasis of direction 3, exponential Euler / ETD2RK (eq. (19), reading R8);
+//               both stages, including the real-space term N(A) (eqs. (9),(11),(16)), happen inside the tile
+//   DOP_COEFF : read only: weighted Gram in real space (C1/D1, rho_tilde) and, after FFT_d, the 1D Parseval sums of
+//               the derivative coefficients  M2_d[a][b] = h^3 A_a^T d_d A_b = (h^3/n) sum k~ (Im a Re b - Re a Im b)
+//
+// Real lines are transformed two at a time as one complex line z = u + i v: all multipliers used here are conjugate
+// symmetric in k (k~ = 0 at Nyquist, reading R4), so Re and Im stay separate lines without any split step.
+//   direction 1: u, v = two consecutive grid rows of the same column (tile = 2L consecutive rows)
+//   direction 2, 3: a double2 of the array (grid points i1 = 2j, 2j+1) already is such a pair (tile = L double2 along i1
+//                   x all points of the line x all columns)
+// Shared layout z[e][line], line = c*L + l fastest (conflict-free butterflies, warp-uniform twiddles); after the
+// forward (decimation-in-frequency) transform element e holds the wavenumber of bit-reversed position e, and all
+// tables are stored in that order.
+#pragma once
+#include "common.cuh"
+
+enum { DOP_EXACT = 0, DOP_ETD1 = 1, DOP_ETD2 = 2, DOP_COEFF = 3 };
+enum { DW_NONE = 0, DW_E = 1, DW_V = 2 };
+
+struct DirArgs {
+    GridDev g;
+    const double* in;      // N x R real, column stride N
+    double* out;           // N x R real (may alias in)
+    const double* E;       // [3][N] electric field (DW_E)
+    const double* min_;    // [R][R] ([cin][cout]) applied at load, or nullptr
+    const double* mout;    // [R][R] applied before the store, or nullptr
+    const double* Q;       // 3 x [R][R]: real-space term in the eigenbasis, G = sum_i w_i o (m Q_i)
+    const double2* ph;     // [n][R] EXACT: phases by stored position
+    const double2 *ez, *f1, *f2a, *f2b;   // [n][R] ETD: e^z, t phi1, t (phi1 - phi2), t phi2
+    double* gram;          // per-CTA partial sums: plain Gram of the OUTPUT (EXACT/ETD), weighted Gram of the INPUT (COEFF)
+    double* pgram;         // COEFF: per-CTA Parseval partial sums [grid][R(R-1)/2]
+    double* colsum;        // per-CTA column sums of the output [grid][R], or nullptr
+    int L;                 // packed lines per column in a tile (power of two)
+    int store;             // write `out`
+    int threads;           // CTA size (0 = DLR_THREADS)
+};
+
+__host__ __device__ inline int dir_tiles(int n, int L) { return (n * n / 2) / L; }     // same count for all directions
+
+__host__ inline size_t dir_smem_bytes(int n, int R, int L, int nbuf, int nmat, bool needE) {
+    const int LP = (nbuf * R * L) | 1;
+    size_t b = (size_t)n * LP * 16 + (size_t)(n / 2) * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
+    if (needE) b += (size_t)3 * n * L * 16;
+    return b + 16;
+}
+
+// tile position
+struct DirGeom {
+    int n, lg, M, L, lL;
+    int q0;          // DIR 1: first row
+    int ia;          // DIR 2: i3 of the tile;  DIR 3: i2 of the tile
+    int j0;          // DIR 2, 3: first double2 along i1
+    double lo, h;
+};
+
+// global double2 index (within one column) of tile element (e, l); DIR 1 returns the index of row u (row v is + M)
+template <int DIR>
+__device__ __forceinline__ size_t dir_index(const DirGeom& gm, int e, int l) {
+    if (DIR == 1) return (size_t)(gm.q0 + 2 * l) * gm.M + e;                      // e = double2 index j along the row
+    if (DIR == 2) return ((size_t)((gm.ia << gm.lg) + e)) * gm.M + gm.j0 + l;     // (i3*n + i2)*M + j
+    return ((size_t)((e << gm.lg) + gm.ia)) * gm.M + gm.j0 + l;                   // (i3*n + i2)*M + j
+}
+
+// weights of the three real-space terms at the two grid points packed in element (e, l): .x for Re, .y for Im
+template <int DIR, int DW>
+__device__ __forceinline__ void dir_weights(const DirGeom& gm, const double2* Et, int e, int l, double2& w0,
+                                            double2& w1, double2& w2) {
+    if (DW == DW_E) {
+        const int nL = gm.n * gm.L;
+        const double2* p = Et + e * gm.L + l;
+        w0 = p[0]; w1 = p[nL]; w2 = p[2 * nL];
+    } else {
+        if (DIR == 1) {
+            const int q = gm.q0 + 2 * l, i2 = q & (gm.n - 1), i3 = q >> gm.lg;
+            const double x1 = gm.lo + gm.h * e;
+            w0 = make_double2(x1, x1);
+            w1 = make_double2(gm.lo + gm.h * i2, gm.lo + gm.h * (i2 + 1));
+            const double x3 = gm.lo + gm.h * i3;
+            w2 = make_double2(x3, x3);
+        } else {
+            const int i1 = 2 * (gm.j0 + l);
+            w0 = make_double2(gm.lo + gm.h * i1, gm.lo + gm.h * (i1 + 1));
+            const double xe = gm.lo + gm.h * e, xa = gm.lo + gm.h * gm.ia;
+            if (DIR == 2) { w1 = make_double2(xe, xe); w2 = make_double2(xa, xa); }
+            else { w1 = make_double2(xa, xa); w2 = make_double2(xe, xe); }
+        }
+    }
+}
+
+template <int R>
+__device__ __forceinline__ void dir_matvec(double2 (&x)[R], const double* A) {     // x <- x * A, A[cin][cout]
+    double2 y[R];
+#pragma unroll
+    for (int co = 0; co < R; co++) {
+        double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int ci = 0; ci < R; ci++) {
+            const double m = A[ci * R + co];
+            acc.x = fma(m, x[ci].x, acc.x);
+            acc.y = fma(m, x[ci].y, acc.y);
+        }
+        y[co] = acc;
+    }
+#pragma unroll
+    for (int c = 0; c < R; c++) x[c] = y[c];
+}
+
+// real-space term in the eigenbasis: g = sum_i w_i o (m Q_i), component co written to gout[co * stride]
+// (streamed out one component at a time: only m stays in registers)
+template <int R>
+__device__ __forceinline__ void dir_nonlin(const double2 (&m)[R], double2* gout, int stride, const double* Q, double2 w0,
+                                           double2 w1, double2 w2) {
+#pragma unroll
+    for (int co = 0; co < R; co++) {
+        double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
+#pragma unroll
+        for (int ci = 0; ci < R; ci++) {
+            const double q0 = Q[ci * R + co], q1 = Q[R * R + ci * R + co], q2 = Q[2 * R * R + ci * R + co];
+            s0.x = fma(q0, m[ci].x, s0.x); s0.y = fma(q0, m[ci].y, s0.y);
+            s1.x = fma(q1, m[ci].x, s1.x); s1.y = fma(q1, m[ci].y, s1.y);
+            s2.x = fma(q2, m[ci].x, s2.x); s2.y = fma(q2, m[ci].y, s2.y);
+        }
+        gout[co * stride] = make_double2(fma(w0.x, s0.x, fma(w1.x, s1.x, w2.x * s2.x)),
+                                         fma(w0.y, s0.y, fma(w1.y, s1.y, w2.y * s2.y)));
+    }
+}
+
+// Gram sums over a tile, one warp per entry (fixed order, no atomics).
+//   DW_NONE: plain  part[pe] = sum a.b                                  (P = R(R+1)/2 upper pairs)
+//   DW_E/V : part[d*P + pe] = sum w_d a.b, d = 0..2;  COLSUM: part[3P + c] = sum a_c
+template <int R, int DIR, int DW, bool COLSUM>
+__device__ __forceinline__ void dir_gram(const double2* z, int LPZ, const DirGeom& gm, const double2* Et, double* part) {
+    constexpr int P = R * (R + 1) / 2;
+    constexpr int NENT = COLSUM ? P + R : P;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+    const int items = gm.n * gm.L;
+    for (int en = warp; en < NENT; en += nwarp) {
+        int ca = 0, cb = 0;
+        if (en < P) {
+            int rem = en;
+            while (rem >= R - ca) { rem -= R - ca; ca++; }
+            cb = ca + rem;
+        } else {
+            ca = cb = en - P;
+        }
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+        for (int w = lane; w < items; w += 32) {
+            const int l = w & (gm.L - 1), e = w >> gm.lL;
+            const double2 za = z[(size_t)e * LPZ + ca * gm.L + l];
+            if (en >= P) { s0 += za.x + za.y; continue; }
+            const double2 zb = z[(size_t)e * LPZ + cb * gm.L + l];
+            const double px = za.x * zb.x, py = za.y * zb.y;
+            if (DW == DW_NONE) {
+                s0 += px + py;
+            } else {
+                double2 w0, w1, w2;
+                dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
+                s0 = fma(w0.x, px, fma(w0.y, py, s0));
+                s1 = fma(w1.x, px, fma(w1.y, py, s1));
+                s2 = fma(w2.x, px, fma(w2.y, py, s2));
+            }
+        }
+        s0 = warp_sum(s0);
+        if (DW != DW_NONE) { s1 = warp_sum(s1); s2 = warp_sum(s2); }
+        if (lane == 0) {
+            if (DW == DW_NONE) part[en] = s0;
+            else if (en < P) { part[en] = s0; part[P + en] = s1; part[2 * P + en] = s2; }
+            else part[3 * P + (en - P)] = s0;
+        }
+    }
+}
+
+template <int R, int DIR, int DOP, int DW>
+__global__ void __launch_bounds__(DLR_THREADS, (R <= 10 ? 2 : 1)) k_dir(const DirArgs a) {
+    constexpr bool ETD = (DOP == DOP_ETD1 || DOP == DOP_ETD2);
+    constexpr int NBUF = ETD ? 2 : 1;
+    constexpr int NMAT = ETD ? 5 : 2;
+    constexpr int RR = R * R;
+    const int n = a.g.n, lg = a.g.log2n, M = n >> 1, L = a.L;
+    const int lL = __ffs(L) - 1;
+    const int nl = R * L, LPZ = (NBUF * nl) | 1;
+    extern __shared__ double2 smem2[];
+    double2* z = smem2;                                        // [n][LPZ]
+    double2* tw = z + (size_t)n * LPZ;                         // [n/2]
+    double* mats = (double*)(tw + M);                          // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2
+    double2* Et = (double2*)(mats + ((NMAT * RR + 1) & ~1));   // [3][n][L]
+    const int tid = threadIdx.x, nth = blockDim.x;
+    DirGeom gm;
+    gm.n = n; gm.lg = lg; gm.M = M; gm.L = L; gm.lL = lL; gm.lo = a.g.lo; gm.h = a.g.h;
+    gm.q0 = 0; gm.ia = 0; gm.j0 = 0;
+    if (DIR == 1) {
+        gm.q0 = (int)blockIdx.x * 2 * L;
+    } else {
+        const int ltp = (lg - 1) - lL;                         // log2 of tiles per plane (M / L)
+        gm.ia = (int)blockIdx.x >> ltp;
+        gm.j0 = ((int)blockIdx.x & ((1 << ltp) - 1)) << lL;
+    }
+    for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
+    if (a.min_ != nullptr) for (int i = tid; i < RR; i += nth) mats[i] = a.min_[i];
+    if (a.mout != nullptr) for (int i = tid; i < RR; i += nth) mats[RR + i] = a.mout[i];
+    if (ETD) for (int i = tid; i < 3 * RR; i += nth) mats[2 * RR + i] = a.Q[i];
+    const size_t N2 = (size_t)(a.g.N >> 1);
+    const double invn = 1.0 / (double)n;
+
+    // ------------------------------------------------------------------ load
+    {
+        const double2* in2 = (const double2*)a.in;
+        if (DIR == 1) {
+            const int lM = lg - 1, items = nl << lM;
+            for (int w = tid; w < items; w += nth) {
+                const int j = w & (M - 1), line = w >> lM;
+                const int c = line >> lL, l = line & (L - 1);
+                const double2* p = in2 + (size_t)c * N2 + dir_index<1>(gm, j, l);
+                const double2 ra = p[0], rb = p[M];
+                z[(size_t)(2 * j) * LPZ + line] = make_double2(ra.x, rb.x);
+                z[(size_t)(2 * j + 1) * LPZ + line] = make_double2(ra.y, rb.y);
+            }
+        } else {
+            const int items = nl << lg;
+            for (int w = tid; w < items; w += nth) {
+                const int l = w & (L - 1), e = (w >> lL) & (n - 1), c = w >> (lL + lg);
+                z[(size_t)e * LPZ + c * L + l] = in2[(size_t)c * N2 + dir_index<DIR>(gm, e, l)];
+            }
+        }
+        if (DW == DW_E) {
+            for (int d = 0; d < 3; d++) {
+                const double2* e2 = (const double2*)(a.E + (size_t)d * a.g.N);
+                double2* Ed = Et + (size_t)d * n * L;
+                if (DIR == 1) {
+                    const int lM = lg - 1, items = L << lM;
+                    for (int w = tid; w < items; w += nth) {
+                        const int j = w & (M - 1), l = w >> lM;
+                        const double2* p = e2 + dir_index<1>(gm, j, l);
+                        const double2 ra = p[0], rb = p[M];
+                        Ed[(2 * j) * L + l] = make_double2(ra.x, rb.x);
+                        Ed[(2 * j + 1) * L + l] = make_double2(ra.y, rb.y);
+                    }
+                } else {
+                    const int items = L << lg;
+                    for (int w = tid; w < items; w += nth) {
+                        const int l = w & (L - 1), e = w >> lL;
+                        Ed[e * L + l] = e2[dir_index<DIR>(gm, e, l)];
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    const int pitems = n << lL;                               // tile points (e, l)
+
+    if (DOP == DOP_COEFF) {
+        // -------------------------------------------------------------- coefficients (read only)
+        if (a.gram != nullptr) {
+            constexpr int NV = 3 * (R * (R + 1) / 2) + (DW == DW_V ? R : 0);
+            dir_gram<R, DIR, DW, DW == DW_V>(z, LPZ, gm, Et, a.gram + (size_t)blockIdx.x * NV);
+            __syncthreads();
+        }
+        fft_lines<false>(z, LPZ, nl, lg, tw, 1);
+        constexpr int P2 = R * (R - 1) / 2;
+        const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
+        double* part = a.pgram + (size_t)blockIdx.x * P2;
+        for (int en = warp; en < P2; en += nwarp) {
+            int ca = 0, rem = en;
+            while (rem >= R - 1 - ca) { rem -= R - 1 - ca; ca++; }
+            const int cb = ca + 1 + rem;
+            double s = 0.0;
+            for (int w = lane; w < pitems; w += 32) {
+                const int l = w & (L - 1), e = w >> lL;
+                const double2 za = z[(size_t)e * LPZ + ca * L + l], zb = z[(size_t)e * LPZ + cb * L + l];
+                s = fma(__ldg(a.g.kt2p + e), za.y * zb.x - za.x * zb.y, s);
+            }
+            s = warp_sum(s);
+            if (lane == 0) part[en] = s;
+        }
+        return;
+    }
+
+    if (DOP == DOP_EXACT) {
+        // -------------------------------------------------------------- exact directional sub-flow
+        if (a.min_ != nullptr) {
+            for (int w = tid; w < pitems; w += nth) {
+                const int l = w & (L - 1), e = w >> lL;
+                double2* p = z + (size_t)e * LPZ + l;
+                double2 x[R];
+#pragma unroll
+                for (int c = 0; c < R; c++) x[c] = p[c * L];
+                dir_matvec<R>(x, mats);
+#pragma unroll
+                for (int c = 0; c < R; c++) p[c * L] = x[c];
+            }
+            __syncthreads();
+        }
+        fft_lines<false>(z, LPZ, nl, lg, tw, 1);
+        {
+            const int items = nl << lg;                       // all (e, line)
+            const FastDiv fnl = make_fastdiv((unsigned)nl);
+            for (int w = tid; w < items; w += nth) {
+                const int e = (int)fdiv((unsigned)w, fnl), line = w - e * nl;
+                const int c = line >> lL;
+                double2 ph = __ldg(a.ph + (size_t)e * R + c);
+                ph.x *= invn; ph.y *= invn;
+                double2* p = z + (size_t)e * LPZ + line;
+                *p = cmul(*p, ph);
+            }
+        }
+        __syncthreads();
+        fft_lines<true>(z, LPZ, nl, lg, tw, 1);
+        if (a.mout != nullptr) {
+            for (int w = tid; w < pitems; w += nth) {
+                const int l = w & (L - 1), e = w >> lL;
+                double2* p = z + (size_t)e * LPZ + l;
+                double2 x[R];
+#pragma unroll
+                for (int c = 0; c < R; c++) x[c] = p[c * L];
+                dir_matvec<R>(x, mats + RR);
+#pragma unroll
+                for (int c = 0; c < R; c++) p[c * L] = x[c];
+            }
+            __syncthreads();
+        }
+    }
+
+    if (ETD) {
+        // -------------------------------------------------------------- third sub-flow, exponential Runge-Kutta
+        const double* Q = mats + 2 * RR;
+        for (int w = tid; w < pitems; w += nth) {             // m = A Min,  g0 = N'(m)
+            const int l = w & (L - 1), e = w >> lL;
+            double2* p = z + (size_t)e * LPZ + l;
+            double2 x[R];
+#pragma unroll
+            for (int c = 0; c < R; c++) x[c] = p[c * L];
+            if (a.min_ != nullptr) {
+                dir_matvec<R>(x, mats);
+#pragma unroll
+                for (int c = 0; c < R; c++) p[c * L] = x[c];
+            }
+            double2 w0, w1, w2;
+            dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
+            dir_nonlin<R>(x, p + nl, L, Q, w0, w1, w2);
+        }
+        __syncthreads();
+        fft_lines<false>(z, LPZ, 2 * nl, lg, tw, 1);
+        {
+            const int items = nl << lg;
+            const FastDiv fnl = make_fastdiv((unsigned)nl);
+            for (int w = tid; w < items; w += nth) {
+                const int e = (int)fdiv((unsigned)w, fnl), line = w - e * nl;
+                const int c = line >> lL;
+                double2* p = z + (size_t)e * LPZ + line;
+                const double2 Mh = p[0], Gh = p[nl];
+                const double2 em = cmul(Mh, __ldg(a.ez + (size_t)e * R + c));
+                const double2 ah = cadd(em, cmul(Gh, __ldg(a.f1 + (size_t)e * R + c)));
+                if (DOP == DOP_ETD1) {
+                    p[0] = ah;
+                } else {
+                    p[nl] = ah;                               // a^ (stage-1 state), inverse-transformed for N'(a)
+                    p[0] = cadd(em, cmul(Gh, __ldg(a.f2a + (size_t)e * R + c)));
+                }
+            }
+        }
+        __syncthreads();
+        if (DOP == DOP_ETD2) {
+            fft_lines<true>(z + nl, LPZ, nl, lg, tw, 1);
+            for (int w = tid; w < pitems; w += nth) {         // g1 = N'(a)
+                const int l = w & (L - 1), e = w >> lL;
+                double2* p = z + (size_t)e * LPZ + nl + l;
+                double2 x[R];
+#pragma unroll
+                for (int c = 0; c < R; c++) { x[c] = p[c * L]; x[c].x *= invn; x[c].y *= invn; }
+                double2 w0, w1, w2;
+                dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
+                dir_nonlin<R>(x, p, L, Q, w0, w1, w2);            // x is fully in registers: in-place is safe
+            }
+            __syncthreads();
+            fft_lines<false>(z + nl, LPZ, nl, lg, tw, 1);
+            {
+                const int items = nl << lg;
+                const FastDiv fnl = make_fastdiv((unsigned)nl);
+                for (int w = tid; w < items; w += nth) {
+                    const int e = (int)fdiv((unsigned)w, fnl), line = w - e * nl;
+                    const int c = line >> lL;
+                    double2* p = z + (size_t)e * LPZ + line;
+                    p[0] = cadd(p[0], cmul(p[nl], __ldg(a.f2b + (size_t)e * R + c)));
+                }
+            }
+            __syncthreads();
+        }
+        fft_lines<true>(z, LPZ, nl, lg, tw, 1);
+        for (int w = tid; w < pitems; w += nth) {             // scale of the inverse transform, back to the output basis
+            const int l = w & (L - 1), e = w >> lL;
+            double2* p = z + (size_t)e * LPZ + l;
+            double2 x[R];
+#pragma unroll
+            for (int c = 0; c < R; c++) { x[c] = p[c * L]; x[c].x *= invn; x[c].y *= invn; }
+            if (a.mout != nullptr) dir_matvec<R>(x, mats + RR);
+#pragma unroll
+            for (int c = 0; c < R; c++) p[c * L] = x[c];
+        }
+        __syncthreads();
+    }
+
+    // ------------------------------------------------------------------ sums of the output, store
+    if (a.gram != nullptr)
+        dir_gram<R, DIR, DW_NONE, false>(z, LPZ, gm, Et, a.gram + (size_t)blockIdx.x * (R * (R + 1) / 2));
+    if (a.colsum != nullptr) {
+        const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
+        for (int c = warp; c < R; c += nwarp) {
+            double s = 0.0;
+            for (int w = lane; w < pitems; w += 32) {
+                const double2 v = z[(size_t)(w >> lL) * LPZ + c * L + (w & (L - 1))];
+                s += v.x + v.y;
+            }
+            s = warp_sum(s);
+            if (lane == 0) a.colsum[(size_t)blockIdx.x * R + c] = s;
+        }
+    }
+    if (a.store) {
+        double2* out2 = (double2*)a.out;
+        if (DIR == 1) {
+            const int lM = lg - 1, items = nl << lM;
+            for (int w = tid; w < items; w += nth) {
+                const int j = w & (M - 1), line = w >> lM;
+                const int c = line >> lL, l = line & (L - 1);
+                const double2 za = z[(size_t)(2 * j) * LPZ + line], zb = z[(size_t)(2 * j + 1) * LPZ + line];
+                double2* p = out2 + (size_t)c * N2 + dir_index<1>(gm, j, l);
+                p[0] = make_double2(za.x, zb.x);
+                p[M] = make_double2(za.y, zb.y);
+            }
+        } else {
+            const int items = nl << lg;
+            for (int w = tid; w < items; w += nth) {
+                const int l = w & (L - 1), e = (w >> lL) & (n - 1), c = w >> (lL + lg);
+                out2[(size_t)c * N2 + dir_index<DIR>(gm, e, l)] = z[(size_t)e * LPZ + c * L + l];
+            }
+        }
+    }
+}
+
+template <int R, int DIR, int DOP, int DW>
+inline cudaError_t launch_dir(const DirArgs& a, cudaStream_t st) {
+    constexpr bool ETD = (DOP == DOP_ETD1 || DOP == DOP_ETD2);
+    auto kern = k_dir<R, DIR, DOP, DW>;
+    const size_t sm = dir_smem_bytes(a.g.n, R, a.L, ETD ? 2 : 1, ETD ? 5 : 2, DW == DW_E);
+    static size_t configured = 0;
+    if (sm > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        if (e != cudaSuccess) return e;
+        configured = sm;
+    }
+    kern<<<(unsigned)dir_tiles(a.g.n, a.L), a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
+    return cudaGetLastError();
+}

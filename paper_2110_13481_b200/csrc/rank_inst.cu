@@ -15,26 +15,22 @@ extern "C" const RankOps* CAT(dlr_rank_ops_, DLR_RANK)() {
     static const RankOps ops = {
         R,
         {
-            launch_d1<R, R, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>,
-            launch_d1<R, R, D1_IN_REAL, D1_OP_NONE, D1_GRAM_V, D1_OUT_CPLX>,
-            launch_d1<R, R, D1_IN_REAL, D1_OP_NONE, D1_GRAM_E, D1_OUT_CPLX>,
-            launch_d1<R, R, D1_IN_CPLX, D1_OP_NONLIN_E, D1_GRAM_NONE, D1_OUT_CPLX>,
-            launch_d1<R, R, D1_IN_CPLX, D1_OP_NONLIN_V, D1_GRAM_NONE, D1_OUT_CPLX>,
-            launch_d1<R, R, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_PLAIN, D1_OUT_REAL>,
-            launch_d1<R, R, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>,
             launch_d1<R, R, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_PLAIN, D1_OUT_REAL>,
             launch_d1<R, R, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_NONE, D1_OUT_REAL>,
             launch_d1<R, R, D1_IN_REAL, D1_OP_NONE, D1_GRAM_PLAIN, D1_OUT_NONE>,
             launch_d1<R, 1, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_NONE, D1_OUT_CPLX>,
         },
         {
-            launch_d3<R, R, D3_FWD_STORE, false>,
-            launch_d3<R, R, D3_FWD_STORE, true>,
-            launch_d3<R, R, D3_FLOW_START, false>,
-            launch_d3<R, R, D3_EULER_END, false>,
-            launch_d3<R, R, D3_MID, false>,
-            launch_d3<R, R, D3_END2, false>,
-            launch_d3<R, R, D3_INV_ONLY, false>,
+            launch_dir<R, 1, DOP_EXACT, DW_NONE>,
+            launch_dir<R, 2, DOP_EXACT, DW_NONE>,
+            launch_dir<R, 3, DOP_ETD1, DW_E>,
+            launch_dir<R, 3, DOP_ETD1, DW_V>,
+            launch_dir<R, 3, DOP_ETD2, DW_E>,
+            launch_dir<R, 3, DOP_ETD2, DW_V>,
+            launch_dir<R, 1, DOP_COEFF, DW_V>,
+            launch_dir<R, 1, DOP_COEFF, DW_E>,
+            launch_dir<R, 2, DOP_COEFF, DW_NONE>,
+            launch_dir<R, 3, DOP_COEFF, DW_NONE>,
         }};
     return &ops;
 }

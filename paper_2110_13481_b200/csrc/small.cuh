@@ -193,9 +193,9 @@ __device__ inline void phi12_imag(double th, double2& p1, double2& p2) {
 // sgn = -1 (K equation (9)) or +1 (L equation (11)); tsub = length of sub-flows 1,2; t3 = length of sub-flow 3.
 // M2c: 3 x [R][R] derivative coefficients; nl gets nlsign * M2c (matrices of the real-space term).
 struct FlowTabPtrs {
-    double* mats;   // 8 R^2
-    double* nl;     // 3 R^2
-    double2 *ph1, *ph2, *ez, *f1, *f2a, *f2b;
+    double* mats;   // 8 R^2: 0 Sin*T1, 1 T1^T T2, 2 T2^T T3, 3 T3^T, 4 T3, 5 T3^T T2, 6 T2^T T1, 7 T1^T  ([cin][cout])
+    double* Q;      // 3 R^2: real-space term in the eigenbasis of direction 3, Q_i = T3^T nl_i^T T3, nl_i = nlsign * M2c_i
+    double2 *ph1, *ph2, *ez, *f1, *f2a, *f2b;   // [n][R] each, by stored (bit-reversed) position
 };
 
 __device__ __forceinline__ void dev_flow_tables(const double* Tm, const double* lam, const double* Sin, int transS,
@@ -224,18 +224,23 @@ __device__ __forceinline__ void dev_flow_tables(const double* Tm, const double* 
         o.mats[5 * RR + idx] = m5;
         o.mats[6 * RR + idx] = m6;
         o.mats[7 * RR + idx] = T1[b * R + a];
-        for (int d = 0; d < 3; d++) o.nl[d * RR + idx] = nlsign * M2c[d * RR + idx];
+        // N(A) T3 = sum_i diag(w_i) (A T3) (T3^T nl_i^T T3):  Q_i[a][b] = sum_pq T3[p][a] nl_i[q][p] T3[q][b]
+        for (int d = 0; d < 3; d++) {
+            double q = 0.0;
+            for (int pp = 0; pp < R; pp++) {
+                double t = 0.0;
+                for (int qq = 0; qq < R; qq++) t = fma(M2c[d * RR + qq * R + pp], T3[qq * R + b], t);
+                q = fma(T3[pp * R + a], t, q);
+            }
+            o.Q[d * RR + idx] = nlsign * q;
+        }
     }
-    const int n = g.n, nh = g.nh;
-    for (int idx = threadIdx.x; idx < nh * R; idx += blockDim.x) {
-        const int k = idx / R, j = idx % R;
-        double sn, cs;
-        sincos(sgn * tsub * g.kt1[k] * lam[j], &sn, &cs);
-        o.ph1[idx] = make_double2(cs, sn);
-    }
+    const int n = g.n;
     for (int idx = threadIdx.x; idx < n * R; idx += blockDim.x) {
         const int k = idx / R, j = idx % R;
         double sn, cs;
+        sincos(sgn * tsub * g.kt2p[k] * lam[j], &sn, &cs);
+        o.ph1[idx] = make_double2(cs, sn);
         sincos(sgn * tsub * g.kt2p[k] * lam[R + j], &sn, &cs);
         o.ph2[idx] = make_double2(cs, sn);
         const double th = sgn * t3 * g.kt2p[k] * lam[2 * R + j];
@@ -304,13 +309,13 @@ __device__ __forceinline__ void dev_sflow(double* S, int R, double t, const doub
 
 // ---------------------------------------------------------------------------------------------------------
 // The r x r work between two streaming phases in ONE launch (single CTA), each part optional:
-//   do_m2 : derivative coefficients M2_i = h^3 A^T d_i A (antisymmetric) from the Parseval partial
-//           sums of the dimension-3 pass: pgram [nblocks][3 P2], entry (a<b) of direction d at d*P2 + pe2;
+//   do_m2 : derivative coefficients M2_i = h^3 A^T d_i A (antisymmetric) from the 1D Parseval
+//           partial sums of the three coefficient passes: pgram[d] [nblocks][P2], entry (a<b) at pe2;
 //   do_s  : S step, one RK4 step of eq. (10);
 //   do_tab: tables of the next K- or L-flow (mode-mixing matrices, phases, phi functions).
 struct PostArgs {
     int R, do_m2, do_s, do_tab;
-    const double* pgram; int nblocks; double m2scale; double* M2;
+    const double* pgram[3]; int nblocks; double m2scale; double* M2;
     double* S; double ts; const double *C1, *C2, *D1, *D2;
     const double *Tm, *lam, *Sin; int transS; GridDev g; double sgn, tsub, t3; const double* M2c; double nlsign;
     FlowTabPtrs o;
@@ -323,7 +328,7 @@ __global__ void __launch_bounds__(DLR_SMALL_THREADS) k_post(const PostArgs a) {
     if (a.do_m2) {
         const int P2 = R * (R - 1) / 2;
         for (int d = 0; d < 3; d++) {
-            cta_reduce_rows(a.pgram, a.nblocks, 3 * P2, d * P2, P2, red, tmp);
+            cta_reduce_rows(a.pgram[d], a.nblocks, P2, 0, P2, red, tmp);
             for (int idx = threadIdx.x; idx < RR; idx += blockDim.x) {
                 const int i = idx / R, j = idx - i * R;
                 double v = 0.0;
@@ -345,6 +350,14 @@ __global__ void __launch_bounds__(DLR_SMALL_THREADS) k_post(const PostArgs a) {
         __syncthreads();
     }
     if (a.do_tab) dev_flow_tables(a.Tm, a.lam, a.Sin, a.transS, R, a.g, a.sgn, a.tsub, a.t3, a.M2c, a.nlsign, a.o);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// column sums of a flow result from the per-CTA sums of its last pass: out[c] = sum_b part[b][c]
+__global__ void __launch_bounds__(DLR_SMALL_THREADS) k_colsum_reduce(const double* part, int nblocks, int R, double* out) {
+    __shared__ double red[DLR_RMAXS], tmp[DLR_SMALL_THREADS];
+    cta_reduce_rows(part, nblocks, R, 0, R, red, tmp);
+    if (threadIdx.x < R) out[threadIdx.x] = red[threadIdx.x];
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -27,7 +27,8 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_config_validation_and_workspace_size(lib):
     from paper_2110_13481_b200 import dlr, inputs
-    for idx, lo, hi in ((1, 1e5, 1e7), (3, 2e8, 1e9), (5, 2.5e10, 6e10)):
+    # about six factor-sized arrays (X, X1, V, KL, Q1, W) plus the field and the r x r work
+    for idx, lo, hi in ((1, 1e5, 1e7), (3, 1.2e8, 5e8), (5, 1.5e10, 4e10)):
         nbytes = dlr.dlr_workspace_bytes(dlr.config_from_inputs(inputs.make_config(idx)))
         assert lo < nbytes < hi
     bad = dlr.make_config(8, 8, 0.0, 1.0, -1.0, 1.0, 5)

@@ -59,15 +59,15 @@ def check(ctx, Xo, So, Vo, gx, gv, ix, iv, tol, e_scale=1.0):
 
 @pytest.mark.parametrize("n,r", [(8, 5), (16, 10), (32, 10), (16, 8), (16, 15), (16, 20)])
 def test_fft_against_numpy(n, r):
-    """the hand-written batched 3D r2c/c2r FFT (three shared-memory passes) against numpy.fft, for the rank-column and
-    the 3-column (field) instantiations; the spectrum is compared in the library's layout (k1 natural 0..n/2,
-    k2/k3 at bit-reversed positions)."""
+    """the hand-written batched 3D r2c/c2r FFT of the Poisson solve (three shared-memory passes, 3 columns) against
+    numpy.fft; the spectrum is compared in the library's layout (k1 natural 0..n/2, k2/k3 at bit-reversed
+    positions).  The 1D transforms inside the K/L-flow passes are covered by the step parity tests below."""
     cfg = inputs.make_config(1, n=n, r=r)
     ctx = make_ctx(cfg)
     rng = np.random.default_rng(n + r)
     lg = int(math.log2(n))
     br = np.array([int(format(i, f"0{lg}b")[::-1], 2) for i in range(n)])
-    for ncols in (r, 3):
+    for ncols in (3,):
         A = np.asfortranarray(rng.standard_normal((n ** 3, ncols)))
         back, spec = ctx.test_fft_roundtrip(0, A)
         ref = np.fft.rfftn(A.T.reshape(ncols, n, n, n), axes=(1, 2, 3))[:, br][:, :, br]
