@@ -99,7 +99,8 @@ int dlr_get_factors(dlr_ctx* ctx, double* X, double* S, double* V, int on_device
 int dlr_get_field(dlr_ctx* ctx, double* E, int on_device);
 
 /* Per-phase device times (ms) of the LAST dlr_step executed with profiling on (dlr_set_profiling(ctx,1)
- * makes dlr_step record CUDA events between phases and disables graph replay). names: the rows of the
+ * makes dlr_step record CUDA events between phases and disables graph replay; on = 2 records an event after every
+ * launch instead, names = the launch expressions). names: the rows of the
  * paper's Table 2. Returns the number of phases written (<= cap). */
 int dlr_set_profiling(dlr_ctx* ctx, int on);
 int dlr_get_phase_times(dlr_ctx* ctx, int cap, float* ms, const char** names);

@@ -42,7 +42,7 @@ struct HostGrid {
     int T2, NB2, nch2;    // dimension-2 pass tiling
     int thr1, thr2, thr3; // CTA sizes of the three pass families
     int Lx, Le, Lc;       // directional passes: packed lines per column for EXACT, ETD and COEFF tiles
-    int thrd;             // CTA size of the directional passes
+    int thrx, thre, thrc; // CTA sizes of the EXACT, ETD and COEFF directional passes
 };
 
 struct FlowTab {
@@ -69,6 +69,8 @@ struct dlr_ctx {
     double2* Eh;
     double *KL, *Q1, *W, *E;
     double *partial, *partialP[3], *partialC, *partial2a;
+    double *gram2, *pgram2[3], *colsum2;     // group sums of the per-CTA partial rows (group_prereduce)
+    unsigned* grp_cnt;                       // 3 x DLR_CNT_STRIDE group counters, zero between kernels
     // small buffers
     double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *zsum, *mx, *mv, *mxp, *mvp, *mres, *esum;
     int* status;
@@ -78,6 +80,7 @@ struct dlr_ctx {
     FlowTab ft;
     double* small_end;
     bool has_state, vh_valid, profiling;
+    int prof_level;               // 1: events between phases; 2: an event after every launch
     int launches, count_launches;
     cudaGraphExec_t graph;
     double graph_tau;
@@ -218,6 +221,11 @@ size_t carve(dlr_ctx* c, char* base) {
     c->partial = cv.take<double>(c->partial_cap);
     for (int d = 0; d < 3; d++) c->partialP[d] = cv.take<double>(blocks * (size_t)(R * (R - 1) / 2));   // Parseval sums
     c->partialC = cv.take<double>(blocks * (size_t)R);                                                  // column sums
+    const size_t groups = (size_t)dlr_groups((int)blocks) + 1;
+    c->gram2 = cv.take<double>(groups * nvmax);
+    for (int d = 0; d < 3; d++) c->pgram2[d] = cv.take<double>(groups * (size_t)(R * (R - 1) / 2));
+    c->colsum2 = cv.take<double>(groups * (size_t)R);
+    c->grp_cnt = cv.take<unsigned>(3 * DLR_CNT_STRIDE);
     c->partial2a = cv.take<double>((size_t)DLR_G1 * nvmax);
     const int RR = R * R;
     c->S = cv.take<double>(RR); c->Sp = cv.take<double>(RR);
@@ -269,7 +277,10 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     hg.thr1 = valid_threads(tune("thr1", DLR_THREADS));
     hg.thr2 = valid_threads(tune("thr2", DLR_THREADS));
     hg.thr3 = valid_threads(tune("thr3", DLR_THREADS));
-    hg.thrd = valid_threads(tune("thrd", DLR_THREADS));
+    auto dthreads = [](int t) { return (t >= 64 && t <= DLR_THREADS && t % 32 == 0) ? t : DLR_THREADS; };
+    hg.thrx = dthreads(tune("thrx", DLR_THREADS));
+    hg.thre = dthreads(tune("thre", DLR_THREADS));
+    hg.thrc = dthreads(tune("thrc", DLR_THREADS));
     const int lmax = 8;
     hg.Lx = choose_L(n, R, 1, 2, false, (size_t)tune("smx", 48) * 1024, lmax);
     hg.Le = choose_L(n, R, 2, 5, true, (size_t)tune("sme", 110) * 1024, lmax);
@@ -318,10 +329,21 @@ cudaError_t upload_tables(dlr_ctx* c, HostGrid& hg, double lo, double hi) {
             c->last_err_msg = std::string(#expr) + ": " + cudaGetErrorString(_e); \
         }                                                             \
         c->count_launches++;                                          \
+        if (c->prof_level == 2) launch_mark(c, #expr);                \
     } while (0)
 
+void launch_mark(dlr_ctx* c, const char* name);
+
 void phase_mark(dlr_ctx* c, const char* name) {
-    if (!c->profiling) return;
+    if (!c->profiling || (c->prof_level == 2 && strcmp(name, "start") != 0)) return;
+    Phase p;
+    p.name = name;
+    cudaEventCreate(&p.ev);
+    cudaEventRecord(p.ev, c->st);
+    c->phases.push_back(p);
+}
+
+void launch_mark(dlr_ctx* c, const char* name) {
     Phase p;
     p.name = name;
     cudaEventCreate(&p.ev);
@@ -335,10 +357,11 @@ void run_d2(dlr_ctx* c, const HostGrid& hg, double2* data, int ncols, bool inv) 
     if (inv) CK(launch_d2<true>(a, c->st)); else CK(launch_d2<false>(a, c->st));
 }
 
-D1Args d1args(const HostGrid& hg) {
+D1Args d1args(dlr_ctx* c, const HostGrid& hg) {
     D1Args a;
     memset(&a, 0, sizeof(a));
     a.g = hg.g; a.T = hg.T1; a.scale = 2.0 / (double)hg.g.N; a.threads = hg.thr1;
+    a.partial2 = c->gram2; a.grp_cnt = c->grp_cnt;
     return a;
 }
 
@@ -358,10 +381,11 @@ void reduce_partials(dlr_ctx* c, int nblocks, int nvals, double* out2) {
 int d1_blocks(const HostGrid& hg) { return (int)((long long)hg.g.n * hg.g.n / hg.T1); }
 int d3_blocks(const HostGrid& hg) { return (int)(((long long)hg.g.nh * hg.g.n + hg.T3 - 1) / hg.T3); }
 
-DirArgs dirargs(const HostGrid& hg) {
+DirArgs dirargs(dlr_ctx* c, const HostGrid& hg) {
     DirArgs a;
     memset(&a, 0, sizeof(a));
-    a.g = hg.g; a.threads = hg.thrd;
+    a.g = hg.g; a.threads = hg.thrx;
+    a.gram2 = c->gram2; a.colsum2 = c->colsum2; a.grp_cnt = c->grp_cnt;
     return a;
 }
 int dir_blocks(const HostGrid& hg, int L) { return dir_tiles(hg.g.n, L); }
@@ -372,21 +396,21 @@ int dir_blocks(const HostGrid& hg, int L) { return dir_tiles(hg.g.n, L); }
 // post(..., do_m2).  M1, its eigen-decomposition (T, lam) and colsum are final when this returns (in stream order).
 void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M1, double* colsum, double* T, double* lam) {
     const int R = c->R;
-    DirArgs a = dirargs(hg);
-    a.in = A; a.E = c->E; a.L = hg.Lc; a.gram = c->partial; a.pgram = c->partialP[0];
+    DirArgs a = dirargs(c, hg);
+    a.in = A; a.E = c->E; a.L = hg.Lc; a.gram = c->partial; a.pgram = c->partialP[0]; a.pgram2 = c->pgram2[0]; a.threads = hg.thrc;
     CK(c->ops->dir[kind == 1 ? VD_COEFF1_V : VD_COEFF1_E](a, c->st));
     // fork: M1 and its eigen-decomposition need only the Gram sums of the pass above; they run beside the two
     // remaining passes (under stream capture this becomes a parallel branch of the step graph)
     CK(cudaEventRecord(c->ev_fork, c->st));
     CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->partial, dir_blocks(hg, hg.Lc), R, kind == 1, hg.g.h3, M1, colsum, T, lam);
+    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->gram2, dlr_groups(dir_blocks(hg, hg.Lc)), R, kind == 1, hg.g.h3, M1, colsum, T, lam);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev_join, c->side));
     c->count_launches -= 3;                         // the three event calls above are not kernel launches
     a.gram = nullptr; a.E = nullptr;
-    a.pgram = c->partialP[1];
+    a.pgram = c->partialP[1]; a.pgram2 = c->pgram2[1];
     CK(c->ops->dir[VD_COEFF2](a, c->st));
-    a.pgram = c->partialP[2];
+    a.pgram = c->partialP[2]; a.pgram2 = c->pgram2[2];
     CK(c->ops->dir[VD_COEFF3](a, c->st));
     CK(cudaStreamWaitEvent(c->st, c->ev_join, 0));  // join before anything reads M1, T, lam, colsum
     c->count_launches -= 1;
@@ -401,8 +425,8 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
     memset(&a, 0, sizeof(a));
     a.R = c->R;
     if (m2) {
-        a.do_m2 = 1; a.nblocks = dir_blocks(*m2->hg, m2->hg->Lc);
-        for (int d = 0; d < 3; d++) a.pgram[d] = c->partialP[d];
+        a.do_m2 = 1; a.nblocks = dlr_groups(dir_blocks(*m2->hg, m2->hg->Lc));
+        for (int d = 0; d < 3; d++) a.pgram[d] = c->pgram2[d];
         a.m2scale = m2->hg->g.h3 / (double)m2->hg->g.n; a.M2 = m2->M2;     // 1D Parseval: sum_x u dv = (1/n) sum_k ...
     }
     if (sf) { a.do_s = 1; a.S = sf->S; a.ts = sf->t; a.C1 = c->C1; a.C2 = c->C2; a.D1 = c->D1; a.D2 = c->D2; }
@@ -410,7 +434,14 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
         a.do_tab = 1; a.Tm = tb->T; a.lam = tb->lam; a.Sin = tb->Sin; a.transS = tb->transS; a.g = tb->hg->g;
         a.sgn = tb->sgn; a.tsub = tb->tsub; a.t3 = tb->t3; a.M2c = tb->M2c; a.nlsign = tb->nlsign; a.o = c->ft.p;
     }
-    k_post<<<1, DLR_SMALL_THREADS, 0, c->st>>>(a);
+    const size_t sm = sf ? (size_t)12 * c->R * c->R * sizeof(double) : 0;     // staged C1, C2, D1, D2
+    static size_t configured = 0;
+    if (sm > configured) {
+        CK(cudaFuncSetAttribute(k_post, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        c->count_launches--;
+        configured = sm;
+    }
+    k_post<<<1, DLR_SMALL_THREADS, sm, c->st>>>(a);
     CK(cudaGetLastError());
 }
 
@@ -419,7 +450,7 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
 // p = scale * S vec (S != nullptr; vec has element stride vstride) or scale * vec is formed inside the first pass.
 void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int vstride, double scale) {
     const HostGrid& hg = c->gx;
-    D1Args a = d1args(hg);
+    D1Args a = d1args(c, hg);
     a.in_real = A; a.out_cplx = c->Eh; a.rho_S = S; a.rho_vec = vec; a.rho_stride = vstride; a.rho_scale = scale;
     CK(c->ops->d1[V1_RHO](a, c->st));
     run_d2(c, hg, c->Eh, 1, false);
@@ -427,7 +458,7 @@ void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int 
     b.in = c->Eh; b.out = c->Eh; b.T = hg.T3s;
     CK((launch_d3<1, 3, D3_POISSON, false>(b, c->st)));
     run_d2(c, hg, c->Eh, 3, true);
-    D1Args e = d1args(hg);
+    D1Args e = d1args(c, hg);
     e.T = hg.T1s; e.in_cplx = c->Eh; e.out_real = c->E;
     CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
 }
@@ -444,10 +475,10 @@ void qr(dlr_ctx* c, const HostGrid& hg, int nblocks0, double* basis, double* Sou
     for (int stage = 0; stage < 3; stage++) {
         // stage 0 reads the Gram sums written by the last pass of the flow (nblocks0 tiles), later stages those of
         // the previous A*Mat pass
-        k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->partial, stage == 0 ? nblocks0 : d1_blocks(hg), R, stage, stage == 2, shift, osc, ssc,
+        k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->gram2, dlr_groups(stage == 0 ? nblocks0 : d1_blocks(hg)), R, stage, stage == 2, shift, osc, ssc,
                                                           transS, c->apply, c->Rtot, Sout, c->status);
         CK(cudaGetLastError());
-        D1Args a = d1args(hg);
+        D1Args a = d1args(c, hg);
         a.in_real = src[stage]; a.out_real = dst[stage]; a.mat = c->apply; a.partial = c->partial;
         CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
     }
@@ -462,7 +493,7 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     const RankOps* ops = c->ops;
     const int RR = c->R * c->R;
     const double* mats = c->ft.p.mats;
-    DirArgs a = dirargs(hg);
+    DirArgs a = dirargs(c, hg);
     a.store = 1; a.L = hg.Lx;
     // sub-flow 1:  A <- src (Sin T1), phases, then into the eigenbasis of direction 2
     a.in = src; a.out = c->W; a.min_ = mats + 0 * RR; a.mout = mats + 1 * RR; a.ph = c->ft.p.ph1;
@@ -471,8 +502,8 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
     CK(ops->dir[VD_EXACT2](a, c->st));
     // sub-flow 3 in the eigenbasis of direction 3
-    DirArgs e = dirargs(hg);
-    e.L = hg.Le; e.in = c->W; e.E = c->E; e.min_ = mats + 2 * RR; e.Q = c->ft.p.Q;
+    DirArgs e = dirargs(c, hg);
+    e.threads = hg.thre; e.L = hg.Le; e.in = c->W; e.E = c->E; e.min_ = mats + 2 * RR; e.Q = c->ft.p.Q;
     e.ez = c->ft.p.ez; e.f1 = c->ft.p.f1; e.f2a = c->ft.p.f2a; e.f2b = c->ft.p.f2b;
     if (order == 1) {
         e.mout = mats + 3 * RR;                      // T3^T: back to the original basis
@@ -480,7 +511,7 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
         else { e.store = 1; e.out = c->KL; e.gram = c->partial; }
         CK(ops->dir[is_L ? VD_ETD1_V : VD_ETD1_E](e, c->st));
         if (zero_only) {
-            k_colsum_reduce<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->partialC, dir_blocks(hg, hg.Le), c->R, c->zsum);
+            k_colsum_reduce<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->colsum2, dlr_groups(dir_blocks(hg, hg.Le)), c->R, c->zsum);
             CK(cudaGetLastError());
         }
         return dir_blocks(hg, hg.Le);
@@ -651,6 +682,7 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     e = upload_tables(c, c->gx, cfg->x_lo[0], cfg->x_hi[0]);
     if (e == cudaSuccess) e = upload_tables(c, c->gv, cfg->v_lo[0], cfg->v_hi[0]);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->status, 0, 4 * sizeof(int), c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->grp_cnt, 0, 3 * DLR_CNT_STRIDE * sizeof(unsigned), c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
     if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
     *out = c;
@@ -670,7 +702,7 @@ void dlr_destroy(dlr_ctx* c) {
 
 static int gram_check(dlr_ctx* c, const HostGrid& hg, const double* A) {
     const int R = c->R, P = R * (R + 1) / 2;
-    D1Args a = d1args(hg);
+    D1Args a = d1args(c, hg);
     a.in_real = A; a.partial = c->partial;
     CK(c->ops->d1[V1_GRAM_ONLY](a, c->st));
     reduce_partials(c, d1_blocks(hg), P, c->partial2a);
@@ -767,6 +799,7 @@ double dlr_bytes_per_step(dlr_ctx* c) {
 int dlr_set_profiling(dlr_ctx* c, int on) {
     if (!c) return DLR_ERR_INVALID;
     c->profiling = on != 0;
+    c->prof_level = on;
     return DLR_OK;
 }
 
@@ -855,11 +888,11 @@ int dlr_test_fft_roundtrip(dlr_ctx* c, int which, int ncols, const double* d_in,
     const HostGrid& hg = which ? c->gv : c->gx;
     if (hg.g.NC > c->gx.g.NC) return DLR_ERR_UNSUPPORTED;      // the scratch spectrum is sized for the x grid
     double2* spec = (double2*)d_spec;
-    D1Args a = d1args(hg);
+    D1Args a = d1args(c, hg);
     a.in_real = d_in; a.out_cplx = spec; a.T = hg.T1s;
     D3Args b = d3args(c, hg);
     b.in = spec; b.out = spec; b.T = hg.T3s;
-    D1Args e = d1args(hg);
+    D1Args e = d1args(c, hg);
     e.in_cplx = spec; e.out_real = d_out; e.T = hg.T1s;
     CK((launch_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>(a, c->st)));
     run_d2(c, hg, spec, ncols, false);

@@ -139,6 +139,32 @@ __device__ __forceinline__ void fft_lines(double2* s, int LP, int nlines, int lo
     }
 }
 
+// ---------------------------------------------------------------- two-level deterministic partial sums
+// A producer CTA writes its partial row rows[blockIdx.x][0..nvals); the LAST CTA to finish of every group of DLR_GRP
+// consecutive CTAs then adds the group's rows in index order into rows2[group][0..nvals).  The result does not depend
+// on which CTA does it, so the sums stay bit-reproducible; the single-CTA consumer only reads gridDim.x / DLR_GRP
+// rows.  counters[group] must be 0 on entry and is 0 again on exit (atomicInc wraps).
+#define DLR_GRP 16
+__host__ __device__ inline int dlr_groups(int nblocks) { return (nblocks + DLR_GRP - 1) / DLR_GRP; }
+
+__device__ __forceinline__ void group_prereduce(const double* rows, int nvals, unsigned* counters, double* rows2) {
+    __shared__ int s_last;
+    __threadfence();
+    __syncthreads();
+    const int grp = (int)blockIdx.x / DLR_GRP, first = grp * DLR_GRP;
+    const int cnt = min(DLR_GRP, (int)gridDim.x - first);
+    if (threadIdx.x == 0) s_last = (atomicInc(counters + grp, (unsigned)(cnt - 1)) == (unsigned)(cnt - 1));
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int v = threadIdx.x; v < nvals; v += blockDim.x) {
+        const double* p = rows + (size_t)first * nvals + v;
+        double s = 0.0;
+        for (int b = 0; b < cnt; b++) s += __ldcg(p + (size_t)b * nvals);     // L2 (other CTAs wrote these)
+        rows2[(size_t)grp * nvals + v] = s;
+    }
+}
+
 __device__ __forceinline__ int brev(int k, int logM) { return (int)(__brev((unsigned)k) >> (32 - logM)); }
 
 // ---------------------------------------------------------------- warp-owned Gram accumulation

@@ -23,6 +23,8 @@ struct D1Args {
     const double* mat;         // MATVEC: [RIN][ROUT];  NONLIN: 3 x [R][R], out_c = sum_i w_i sum_c' M_i[c][c'] a_c'
     const double* E;           // [3][N] weights for NONLIN_E / GRAM_E
     double* partial;           // [gridDim.x][nvals] Gram partial sums
+    double* partial2;          // [groups][nvals] group sums (see group_prereduce), or nullptr
+    unsigned* grp_cnt;         // group counters
     double scale;              // applied to the data after a complex input (2/N for an inverse transform)
     int T;                     // rows per CTA (power of two dividing n^2)
     int threads;               // CTA size (0 = DLR_THREADS)
@@ -232,6 +234,7 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     }
 
     // ------------------------------------------------------------------ store
+    // (the group sums of the Gram rows are formed after the store so that the fence covers only small data)
     if (OUT_MODE & D1_OUT_REAL) {
         const int cnt = T * M;
         for (int c = 0; c < ROUT; c++) {
@@ -261,6 +264,8 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
             if (k != M - k) row[M - k] = cconj(csub(ze, wz));
         }
     }
+    if (GRAM != D1_GRAM_NONE && a.partial2 != nullptr)
+        group_prereduce(a.partial, d1_gram_nvals(ROUT, GRAM), a.grp_cnt, a.partial2);
 }
 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>

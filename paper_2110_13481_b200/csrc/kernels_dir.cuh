@@ -22,6 +22,7 @@
 
 enum { DOP_EXACT = 0, DOP_ETD1 = 1, DOP_ETD2 = 2, DOP_COEFF = 3 };
 enum { DW_NONE = 0, DW_E = 1, DW_V = 2 };
+#define DLR_CNT_STRIDE 4096
 
 struct DirArgs {
     GridDev g;
@@ -36,6 +37,8 @@ struct DirArgs {
     double* gram;          // per-CTA partial sums: plain Gram of the OUTPUT (EXACT/ETD), weighted Gram of the INPUT (COEFF)
     double* pgram;         // COEFF: per-CTA Parseval partial sums [grid][R(R-1)/2]
     double* colsum;        // per-CTA column sums of the output [grid][R], or nullptr
+    double *gram2, *pgram2, *colsum2;   // group sums of the three (see group_prereduce)
+    unsigned* grp_cnt;     // group counters: [0..) gram, [DLR_CNT_STRIDE..) pgram, [2 DLR_CNT_STRIDE..) colsum
     int L;                 // packed lines per column in a tile (power of two)
     int store;             // write `out`
     int threads;           // CTA size (0 = DLR_THREADS)
@@ -177,8 +180,11 @@ __device__ __forceinline__ void dir_gram(const double2* z, int LPZ, const DirGeo
 }
 
 template <int R, int DIR, int DOP, int DW>
-__global__ void __launch_bounds__(DLR_THREADS, (R <= 10 ? 2 : 1)) k_dir(const DirArgs a) {
+__global__ void __launch_bounds__(DLR_THREADS, ((DOP == DOP_EXACT && DIR == 2) ? (R <= 10 ? 4 : 2) : (R <= 10 ? 2 : 1)))
+k_dir(const DirArgs a) {
     constexpr bool ETD = (DOP == DOP_ETD1 || DOP == DOP_ETD2);
+    constexpr bool MIX = ETD || (DOP == DOP_EXACT && DIR == 1);   // column mixing exists only in these passes: the
+                                                                  // direction-2 sub-flow keeps a small register budget
     constexpr int NBUF = ETD ? 2 : 1;
     constexpr int NMAT = ETD ? 5 : 2;
     constexpr int RR = R * R;
@@ -202,8 +208,8 @@ __global__ void __launch_bounds__(DLR_THREADS, (R <= 10 ? 2 : 1)) k_dir(const Di
         gm.j0 = ((int)blockIdx.x & ((1 << ltp) - 1)) << lL;
     }
     for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
-    if (a.min_ != nullptr) for (int i = tid; i < RR; i += nth) mats[i] = a.min_[i];
-    if (a.mout != nullptr) for (int i = tid; i < RR; i += nth) mats[RR + i] = a.mout[i];
+    if (MIX && a.min_ != nullptr) for (int i = tid; i < RR; i += nth) mats[i] = a.min_[i];
+    if (MIX && a.mout != nullptr) for (int i = tid; i < RR; i += nth) mats[RR + i] = a.mout[i];
     if (ETD) for (int i = tid; i < 3 * RR; i += nth) mats[2 * RR + i] = a.Q[i];
     const size_t N2 = (size_t)(a.g.N >> 1);
     const double invn = 1.0 / (double)n;
@@ -278,12 +284,17 @@ __global__ void __launch_bounds__(DLR_THREADS, (R <= 10 ? 2 : 1)) k_dir(const Di
             s = warp_sum(s);
             if (lane == 0) part[en] = s;
         }
+        if (a.gram != nullptr) {
+            constexpr int NV = 3 * (R * (R + 1) / 2) + (DW == DW_V ? R : 0);
+            group_prereduce(a.gram, NV, a.grp_cnt, a.gram2);
+        }
+        group_prereduce(a.pgram, P2, a.grp_cnt + DLR_CNT_STRIDE, a.pgram2);
         return;
     }
 
     if (DOP == DOP_EXACT) {
         // -------------------------------------------------------------- exact directional sub-flow
-        if (a.min_ != nullptr) {
+        if (MIX && a.min_ != nullptr) {
             for (int w = tid; w < pitems; w += nth) {
                 const int l = w & (L - 1), e = w >> lL;
                 double2* p = z + (size_t)e * LPZ + l;
@@ -311,7 +322,7 @@ __global__ void __launch_bounds__(DLR_THREADS, (R <= 10 ? 2 : 1)) k_dir(const Di
         }
         __syncthreads();
         fft_lines<true>(z, LPZ, nl, lg, tw, 1);
-        if (a.mout != nullptr) {
+        if (MIX && a.mout != nullptr) {
             for (int w = tid; w < pitems; w += nth) {
                 const int l = w & (L - 1), e = w >> lL;
                 double2* p = z + (size_t)e * LPZ + l;
@@ -440,6 +451,8 @@ __global__ void __launch_bounds__(DLR_THREADS, (R <= 10 ? 2 : 1)) k_dir(const Di
             }
         }
     }
+    if (a.gram != nullptr) group_prereduce(a.gram, R * (R + 1) / 2, a.grp_cnt, a.gram2);
+    if (a.colsum != nullptr) group_prereduce(a.colsum, R, a.grp_cnt + 2 * DLR_CNT_STRIDE, a.colsum2);
 }
 
 template <int R, int DIR, int DOP, int DW>

@@ -40,16 +40,14 @@ __device__ __forceinline__ void cta_reduce_rows(const double* __restrict__ parti
     const int g = tid / nvals, v = tid - g * nvals;
     if (g < G) {
         const double* p = partial + off + v;
-        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        double s[8] = {0, 0, 0, 0, 0, 0, 0, 0};          // eight loads in flight per thread, fixed summation order
         int b = g;
-        for (; b + 3 * G < nblocks; b += 4 * G) {
-            s0 += p[(size_t)b * stride];
-            s1 += p[(size_t)(b + G) * stride];
-            s2 += p[(size_t)(b + 2 * G) * stride];
-            s3 += p[(size_t)(b + 3 * G) * stride];
+        for (; b + 7 * G < nblocks; b += 8 * G) {
+#pragma unroll
+            for (int u = 0; u < 8; u++) s[u] += p[(size_t)(b + u * G) * stride];
         }
-        for (; b < nblocks; b += G) s0 += p[(size_t)b * stride];
-        tmp[g * nvals + v] = (s0 + s1) + (s2 + s3);
+        for (; b < nblocks; b += G) s[0] += p[(size_t)b * stride];
+        tmp[g * nvals + v] = ((s[0] + s[1]) + (s[2] + s[3])) + ((s[4] + s[5]) + (s[6] + s[7]));
     }
     __syncthreads();
     if (tid < nvals) {
@@ -162,19 +160,21 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
 // ---------------------------------------------------------------------------------------------------------
 // phi functions of a purely imaginary argument z = i*theta (reading R7): closed forms for |theta| >= 1,
 // Taylor series below.
+__device__ const double DLR_INV_FACT[24] = {      // 1/k!, k = 1..24 (correctly rounded)
+    1.0, 0.5, 0.16666666666666666, 0.041666666666666664,
+    0.008333333333333333, 0.001388888888888889, 0.0001984126984126984, 2.48015873015873e-05,
+    2.7557319223985893e-06, 2.755731922398589e-07, 2.505210838544172e-08, 2.08767569878681e-09,
+    1.6059043836821613e-10, 1.1470745597729725e-11, 7.647163731819816e-13, 4.779477332387385e-14,
+    2.8114572543455206e-15, 1.5619206968586225e-16, 8.22063524662433e-18, 4.110317623312165e-19,
+    1.9572941063391263e-20, 8.896791392450574e-22, 3.868170170630684e-23, 1.6117375710961184e-24};
 __device__ inline void phi12_imag(double th, double2& p1, double2& p2) {
     if (fabs(th) < 1.0) {
         // Horner in z = i th:  phi1 = sum z^m/(m+1)!,  phi2 = sum z^m/(m+2)!
         double2 s1 = make_double2(0.0, 0.0), s2 = s1;
-        double f1 = 1.0, f2 = 1.0;             // 1/(m+1)!, 1/(m+2)! built on the fly
-        double inv[24];
-        double fac = 1.0;
-        for (int m = 0; m < 24; m++) { fac *= (double)(m + 1); inv[m] = 1.0 / fac; }   // inv[m] = 1/(m+1)!
-        (void)f1; (void)f2;
         for (int m = 21; m >= 0; m--) {
             // s = s*z + coeff,  z = (0, th)
-            s1 = make_double2(-s1.y * th + inv[m], s1.x * th);
-            s2 = make_double2(-s2.y * th + inv[m + 1], s2.x * th);
+            s1 = make_double2(-s1.y * th + DLR_INV_FACT[m], s1.x * th);
+            s2 = make_double2(-s2.y * th + DLR_INV_FACT[m + 1], s2.x * th);
         }
         p1 = s1; p2 = s2;
     } else {
@@ -200,7 +200,8 @@ struct FlowTabPtrs {
 
 __device__ __forceinline__ void dev_flow_tables(const double* Tm, const double* lam, const double* Sin, int transS,
                                                 int R, const GridDev& g, double sgn, double tsub, double t3,
-                                                const double* M2c, double nlsign, const FlowTabPtrs& o) {
+                                                const double* M2c, double nlsign, const FlowTabPtrs& o,
+                                                double* scratch /* shared, >= 7 R^2 doubles */) {
     const double* T1 = Tm;
     const double* T2 = Tm + R * R;
     const double* T3 = Tm + 2 * R * R;
@@ -224,15 +225,27 @@ __device__ __forceinline__ void dev_flow_tables(const double* Tm, const double* 
         o.mats[5 * RR + idx] = m5;
         o.mats[6 * RR + idx] = m6;
         o.mats[7 * RR + idx] = T1[b * R + a];
-        // N(A) T3 = sum_i diag(w_i) (A T3) (T3^T nl_i^T T3):  Q_i[a][b] = sum_pq T3[p][a] nl_i[q][p] T3[q][b]
-        for (int d = 0; d < 3; d++) {
+    }
+    // N(A) T3 = sum_i diag(w_i) (A T3) (T3^T nl_i^T T3):  Q_i = T3^T (nl_i^T T3), two r^3 products through shared memory
+    {
+        double* T3s = scratch;                 // [R][R]
+        double* nls = scratch + RR;            // 3 x [R][R]
+        double* tmpm = scratch + 4 * RR;       // 3 x [R][R]: nl_i^T T3
+        for (int idx = threadIdx.x; idx < RR; idx += blockDim.x) T3s[idx] = T3[idx];
+        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) nls[idx] = M2c[idx];
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) {
+            const int d = idx / RR, e = idx - d * RR, pp = e / R, b = e - pp * R;
+            double t = 0.0;
+            for (int qq = 0; qq < R; qq++) t = fma(nls[d * RR + qq * R + pp], T3s[qq * R + b], t);
+            tmpm[idx] = t;
+        }
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) {
+            const int d = idx / RR, e = idx - d * RR, a = e / R, b = e - a * R;
             double q = 0.0;
-            for (int pp = 0; pp < R; pp++) {
-                double t = 0.0;
-                for (int qq = 0; qq < R; qq++) t = fma(M2c[d * RR + qq * R + pp], T3[qq * R + b], t);
-                q = fma(T3[pp * R + a], t, q);
-            }
-            o.Q[d * RR + idx] = nlsign * q;
+            for (int pp = 0; pp < R; pp++) q = fma(T3s[pp * R + a], tmpm[d * RR + pp * R + b], q);
+            o.Q[idx] = nlsign * q;
         }
     }
     const int n = g.n;
@@ -345,11 +358,18 @@ __global__ void __launch_bounds__(DLR_SMALL_THREADS) k_post(const PostArgs a) {
         __syncthreads();
     }
     if (a.do_s) {
-        dev_sflow(a.S, R, a.ts, a.C1, a.C2, a.D1, a.D2, sc);
+        // the four coefficient sets go to shared memory in one parallel load: the RK4 loops below are chains of
+        // dependent FMAs and must not wait on global memory
+        extern __shared__ double coef[];                       // [4][3 R^2]: C1, C2, D1, D2
+        const double* src[4] = {a.C1, a.C2, a.D1, a.D2};
+        for (int q = 0; q < 4; q++)
+            for (int i = threadIdx.x; i < 3 * RR; i += blockDim.x) coef[q * 3 * RR + i] = src[q][i];
+        __syncthreads();
+        dev_sflow(a.S, R, a.ts, coef, coef + 3 * RR, coef + 6 * RR, coef + 9 * RR, sc);
         __threadfence_block();
         __syncthreads();
     }
-    if (a.do_tab) dev_flow_tables(a.Tm, a.lam, a.Sin, a.transS, R, a.g, a.sgn, a.tsub, a.t3, a.M2c, a.nlsign, a.o);
+    if (a.do_tab) dev_flow_tables(a.Tm, a.lam, a.Sin, a.transS, R, a.g, a.sgn, a.tsub, a.t3, a.M2c, a.nlsign, a.o, (double*)&sc);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -403,9 +423,10 @@ k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, dou
         if (tid == 0) {
             double sjj = G[j][j];
             if (!(sjj > 1e-30)) { sjj = 1e-30; atomicAdd(status, 1); }     // repaired pivot (counted as a QR fallback)
-            const double dj = sqrt(sjj);
-            U[j][j] = dj;
-            dinv[j] = 1.0 / dj;
+            double ri = rsqrt(sjj);                              // 1/sqrt(pivot), no divide/sqrt chain
+            ri = ri * fma(-0.5 * sjj * ri, ri, 1.5);               // one Newton step (rounding-level accurate)
+            U[j][j] = sjj * ri;
+            dinv[j] = ri;
         }
         __syncthreads();
         if (tid > j && tid < R) U[j][tid] = G[j][tid] * dinv[j];

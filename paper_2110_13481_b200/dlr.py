@@ -180,7 +180,7 @@ class Dlr:
         self._check(lib().dlr_set_profiling(self.h, int(on)), "dlr_set_profiling")
 
     def phase_times(self):
-        cap = 64
+        cap = 512
         ms = (ctypes.c_float * cap)()
         names = (ctypes.c_char_p * cap)()
         n = lib().dlr_get_phase_times(self.h, cap, ms, names)
