@@ -476,10 +476,11 @@ void qr(dlr_ctx* c, const HostGrid& hg, int nblocks0, double* basis, double* Sou
         // stage 0 reads the Gram sums written by the last pass of the flow (nblocks0 tiles), later stages those of
         // the previous A*Mat pass
         k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->gram2, dlr_groups(stage == 0 ? nblocks0 : d1_blocks(hg)), R, stage, stage == 2, shift, osc, ssc,
-                                                          transS, c->apply, c->Rtot, Sout, c->status);
+                                                          transS, c->apply, c->Rtot, Sout, c->status, c->status + 1);
         CK(cudaGetLastError());
         D1Args a = d1args(c, hg);
         a.in_real = src[stage]; a.out_real = dst[stage]; a.mat = c->apply; a.partial = c->partial;
+        if (stage >= 1) { a.skip_flag = c->status + 1; a.skip_mode = stage; a.out_alt = basis; }
         CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
     }
 }

@@ -25,6 +25,9 @@ struct D1Args {
     double* partial;           // [gridDim.x][nvals] Gram partial sums
     double* partial2;          // [groups][nvals] group sums (see group_prereduce), or nullptr
     unsigned* grp_cnt;         // group counters
+    const int* skip_flag;      // adaptive CholeskyQR (see k_chol_stage): if *skip_flag != 0 then
+    int skip_mode;             //   mode 1: write out_alt instead of out_real;  mode 2: the whole launch is a no-op
+    double* out_alt;
     double scale;              // applied to the data after a complex input (2/N for an inverse transform)
     int T;                     // rows per CTA (power of two dividing n^2)
     int threads;               // CTA size (0 = DLR_THREADS)
@@ -65,6 +68,12 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     double* mat = (double*)(tw + M);                          // [NMAT]
     double2* Et = (double2*)(mat + ((NMAT + 1) & ~1));        // [3][M][TP] (pairs of grid points along i1)
     const int tid = threadIdx.x, nth = blockDim.x;
+    double* out_real = a.out_real;
+    bool want_gram = true;
+    if (a.skip_flag != nullptr && *a.skip_flag != 0) {
+        if (a.skip_mode == 2) return;
+        if (a.skip_mode == 1) { out_real = a.out_alt; want_gram = false; }     // this pass is the last one: no Gram
+    }
 
     for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
     if (OP == D1_OP_MATVEC && ROUT == 1 && a.rho_vec != nullptr) {
@@ -183,7 +192,7 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     }
 
     // ------------------------------------------------------------------ Gram accumulation (ROUT columns)
-    if (GRAM != D1_GRAM_NONE) {
+    if (GRAM != D1_GRAM_NONE && want_gram) {
         constexpr int P = ROUT * (ROUT + 1) / 2;
         constexpr int NENT = GRAM == D1_GRAM_V ? P + ROUT : P;      // pairs (+ column sums)
         const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
@@ -238,7 +247,7 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     if (OUT_MODE & D1_OUT_REAL) {
         const int cnt = T * M;
         for (int c = 0; c < ROUT; c++) {
-            double2* dst = (double2*)(a.out_real + (size_t)c * a.g.N) + q0 * M;
+            double2* dst = (double2*)(out_real + (size_t)c * a.g.N) + q0 * M;
             for (int i = tid; i < cnt; i += nth) {
                 const int t = i >> logM, j = i & (M - 1);
                 dst[i] = z[(size_t)j * LP + c * T + t];
@@ -264,7 +273,7 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
             if (k != M - k) row[M - k] = cconj(csub(ze, wz));
         }
     }
-    if (GRAM != D1_GRAM_NONE && a.partial2 != nullptr)
+    if (GRAM != D1_GRAM_NONE && want_gram && a.partial2 != nullptr)
         group_prereduce(a.partial, d1_gram_nvals(ROUT, GRAM), a.grp_cnt, a.partial2);
 }
 

@@ -19,6 +19,7 @@
 // tables are stored in that order.
 #pragma once
 #include "common.cuh"
+#include "fft_reg.cuh"
 
 enum { DOP_EXACT = 0, DOP_ETD1 = 1, DOP_ETD2 = 2, DOP_COEFF = 3 };
 enum { DW_NONE = 0, DW_E = 1, DW_V = 2 };
@@ -48,7 +49,7 @@ __host__ __device__ inline int dir_tiles(int n, int L) { return (n * n / 2) / L;
 
 __host__ inline size_t dir_smem_bytes(int n, int R, int L, int nbuf, int nmat, bool needE) {
     const int LP = (nbuf * R * L) | 1;
-    size_t b = (size_t)n * LP * 16 + (size_t)(n / 2) * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
+    size_t b = (size_t)n * LP * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
     if (needE) b += (size_t)3 * n * L * 16;
     return b + 16;
 }
@@ -193,8 +194,7 @@ k_dir(const DirArgs a) {
     const int nl = R * L, LPZ = (NBUF * nl) | 1;
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                        // [n][LPZ]
-    double2* tw = z + (size_t)n * LPZ;                         // [n/2]
-    double* mats = (double*)(tw + M);                          // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2
+    double* mats = (double*)(z + (size_t)n * LPZ);             // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2
     double2* Et = (double2*)(mats + ((NMAT * RR + 1) & ~1));   // [3][n][L]
     const int tid = threadIdx.x, nth = blockDim.x;
     DirGeom gm;
@@ -207,7 +207,6 @@ k_dir(const DirArgs a) {
         gm.ia = (int)blockIdx.x >> ltp;
         gm.j0 = ((int)blockIdx.x & ((1 << ltp) - 1)) << lL;
     }
-    for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
     if (MIX && a.min_ != nullptr) for (int i = tid; i < RR; i += nth) mats[i] = a.min_[i];
     if (MIX && a.mout != nullptr) for (int i = tid; i < RR; i += nth) mats[RR + i] = a.mout[i];
     if (ETD) for (int i = tid; i < 3 * RR; i += nth) mats[2 * RR + i] = a.Q[i];
@@ -267,7 +266,7 @@ k_dir(const DirArgs a) {
             dir_gram<R, DIR, DW, DW == DW_V>(z, LPZ, gm, Et, a.gram + (size_t)blockIdx.x * NV);
             __syncthreads();
         }
-        fft_lines<false>(z, LPZ, nl, lg, tw, 1);
+        fft_lines_c<false>(z, LPZ, nl, lg, false);
         constexpr int P2 = R * (R - 1) / 2;
         const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
         double* part = a.pgram + (size_t)blockIdx.x * P2;
@@ -307,21 +306,16 @@ k_dir(const DirArgs a) {
             }
             __syncthreads();
         }
-        fft_lines<false>(z, LPZ, nl, lg, tw, 1);
+        fft_lines_c<false>(z, LPZ, nl, lg, true);
         {
-            const int items = nl << lg;                       // all (e, line)
-            const FastDiv fnl = make_fastdiv((unsigned)nl);
-            for (int w = tid; w < items; w += nth) {
-                const int e = (int)fdiv((unsigned)w, fnl), line = w - e * nl;
-                const int c = line >> lL;
-                double2 ph = __ldg(a.ph + (size_t)e * R + c);
-                ph.x *= invn; ph.y *= invn;
-                double2* p = z + (size_t)e * LPZ + line;
-                *p = cmul(*p, ph);
-            }
+            const double2* ph = a.ph;
+            fft_mid(z, LPZ, nl, lg, [&](double2& v, int e, int line) {
+                double2 f = __ldg(ph + (size_t)e * R + (line >> lL));
+                f.x *= invn; f.y *= invn;
+                v = cmul(v, f);
+            });
         }
-        __syncthreads();
-        fft_lines<true>(z, LPZ, nl, lg, tw, 1);
+        fft_lines_c<true>(z, LPZ, nl, lg, true);
         if (MIX && a.mout != nullptr) {
             for (int w = tid; w < pitems; w += nth) {
                 const int l = w & (L - 1), e = w >> lL;
@@ -356,7 +350,7 @@ k_dir(const DirArgs a) {
             dir_nonlin<R>(x, p + nl, L, Q, w0, w1, w2);
         }
         __syncthreads();
-        fft_lines<false>(z, LPZ, 2 * nl, lg, tw, 1);
+        fft_lines_c<false>(z, LPZ, 2 * nl, lg, false);
         {
             const int items = nl << lg;
             const FastDiv fnl = make_fastdiv((unsigned)nl);
@@ -377,7 +371,7 @@ k_dir(const DirArgs a) {
         }
         __syncthreads();
         if (DOP == DOP_ETD2) {
-            fft_lines<true>(z + nl, LPZ, nl, lg, tw, 1);
+            fft_lines_c<true>(z + nl, LPZ, nl, lg, false);
             for (int w = tid; w < pitems; w += nth) {         // g1 = N'(a)
                 const int l = w & (L - 1), e = w >> lL;
                 double2* p = z + (size_t)e * LPZ + nl + l;
@@ -389,7 +383,7 @@ k_dir(const DirArgs a) {
                 dir_nonlin<R>(x, p, L, Q, w0, w1, w2);            // x is fully in registers: in-place is safe
             }
             __syncthreads();
-            fft_lines<false>(z + nl, LPZ, nl, lg, tw, 1);
+            fft_lines_c<false>(z + nl, LPZ, nl, lg, false);
             {
                 const int items = nl << lg;
                 const FastDiv fnl = make_fastdiv((unsigned)nl);
@@ -402,7 +396,7 @@ k_dir(const DirArgs a) {
             }
             __syncthreads();
         }
-        fft_lines<true>(z, LPZ, nl, lg, tw, 1);
+        fft_lines_c<true>(z, LPZ, nl, lg, false);
         for (int w = tid; w < pitems; w += nth) {             // scale of the inverse transform, back to the output basis
             const int l = w & (L - 1), e = w >> lL;
             double2* p = z + (size_t)e * LPZ + l;

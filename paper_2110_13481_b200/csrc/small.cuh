@@ -388,9 +388,14 @@ __global__ void __launch_bounds__(DLR_SMALL_THREADS) k_colsum_reduce(const doubl
 //   apply[ci][co] : matrix for the next A*Mat pass (= D U^-1, times out_scale on the last stage)
 //   Rtot (row-major, upper triangular) accumulates R_stage * Rtot with R_stage = U D^-1.
 //   On the last stage the coupling matrix is written: Sout column-major = Rtot*s_scale (transS=0) or its transpose.
+//   Adaptive third stage: stage 1 holds the Gram matrix of the once-orthogonalised factor; if its largest scaled
+//   off-diagonal entry is < 0.1 the factor after this stage is orthonormal to rounding level (CholeskyQR2 suffices for
+//   kappa(A)^2 u < 1), so stage 1 acts as the last stage and sets qrflag[0] = 1: the stage-1 A*Mat pass then writes
+//   the basis directly and the stage-2 kernels return at once.  Stage 0 clears the flag.
 __global__ void __launch_bounds__(DLR_SMALL_THREADS)
 k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, double shift, double out_scale,
-             double s_scale, int transS, double* apply, double* Rtot, double* Sout, int* status) {
+             double s_scale, int transS, double* apply, double* Rtot, double* Sout, int* status, int* qrflag) {
+    if (stage == 2 && qrflag[0] != 0) return;
     __shared__ double G[DLR_RMAXS][DLR_RMAXS + 1], U[DLR_RMAXS][DLR_RMAXS + 1], Ui[DLR_RMAXS][DLR_RMAXS + 1];
     __shared__ double Rp[DLR_RMAXS][DLR_RMAXS + 1];
     __shared__ double dsc[DLR_RMAXS], sg[DLR_RMAXS], dinv[DLR_RMAXS];
@@ -418,6 +423,22 @@ k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, dou
         Ui[i][j] = 0.0;
     }
     __syncthreads();
+    __shared__ int s_skip;
+    if (threadIdx.x < 32) {                                     // largest off-diagonal entry of the scaled Gram matrix
+        double mx = 0.0;
+        for (int idx = threadIdx.x; idx < RR; idx += 32) {
+            const int i = idx / R, j = idx - i * R;
+            if (i != j) mx = fmax(mx, fabs(G[i][j]));
+        }
+        for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if (threadIdx.x == 0) {
+            s_skip = (stage == 1 && mx < 0.1) ? 1 : 0;
+            if (stage == 0) qrflag[0] = 0;
+            if (stage == 1) qrflag[0] = s_skip;
+        }
+    }
+    __syncthreads();
+    if (s_skip) last = 1;
     // right-looking upper Cholesky G = U^T U
     for (int j = 0; j < R; j++) {
         if (tid == 0) {
