@@ -20,6 +20,7 @@
 #pragma once
 #include "common.cuh"
 #include "fft_reg.cuh"
+#include "gram_mma.cuh"
 
 enum { DOP_EXACT = 0, DOP_ETD1 = 1, DOP_ETD2 = 2, DOP_COEFF = 3 };
 enum { DW_NONE = 0, DW_E = 1, DW_V = 2 };
@@ -47,9 +48,15 @@ struct DirArgs {
 
 __host__ __device__ inline int dir_tiles(int n, int L) { return (n * n / 2) / L; }     // same count for all directions
 
+// double2 elements of the tile region: at least the scratch of the cross-warp MMA reduction (64 doubles per warp)
+__host__ __device__ inline int dir_zelems(int n, int LP) {
+    const int need = (DLR_THREADS / 32) * 64 / 2;
+    return n * LP > need ? n * LP : need;
+}
+
 __host__ inline size_t dir_smem_bytes(int n, int R, int L, int nbuf, int nmat, bool needE) {
     const int LP = (nbuf * R * L) | 1;
-    size_t b = (size_t)n * LP * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
+    size_t b = (size_t)dir_zelems(n, LP) * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
     if (needE) b += (size_t)3 * n * L * 16;
     return b + 16;
 }
@@ -135,49 +142,13 @@ __device__ __forceinline__ void dir_nonlin(const double2 (&m)[R], double2* gout,
     }
 }
 
-// Gram sums over a tile, one warp per entry (fixed order, no atomics).
-//   DW_NONE: plain  part[pe] = sum a.b                                  (P = R(R+1)/2 upper pairs)
-//   DW_E/V : part[d*P + pe] = sum w_d a.b, d = 0..2;  COLSUM: part[3P + c] = sum a_c
-template <int R, int DIR, int DW, bool COLSUM>
-__device__ __forceinline__ void dir_gram(const double2* z, int LPZ, const DirGeom& gm, const double2* Et, double* part) {
-    constexpr int P = R * (R + 1) / 2;
-    constexpr int NENT = COLSUM ? P + R : P;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
-    const int items = gm.n * gm.L;
-    for (int en = warp; en < NENT; en += nwarp) {
-        int ca = 0, cb = 0;
-        if (en < P) {
-            int rem = en;
-            while (rem >= R - ca) { rem -= R - ca; ca++; }
-            cb = ca + rem;
-        } else {
-            ca = cb = en - P;
-        }
-        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-        for (int w = lane; w < items; w += 32) {
-            const int l = w & (gm.L - 1), e = w >> gm.lL;
-            const double2 za = z[(size_t)e * LPZ + ca * gm.L + l];
-            if (en >= P) { s0 += za.x + za.y; continue; }
-            const double2 zb = z[(size_t)e * LPZ + cb * gm.L + l];
-            const double px = za.x * zb.x, py = za.y * zb.y;
-            if (DW == DW_NONE) {
-                s0 += px + py;
-            } else {
-                double2 w0, w1, w2;
-                dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
-                s0 = fma(w0.x, px, fma(w0.y, py, s0));
-                s1 = fma(w1.x, px, fma(w1.y, py, s1));
-                s2 = fma(w2.x, px, fma(w2.y, py, s2));
-            }
-        }
-        s0 = warp_sum(s0);
-        if (DW != DW_NONE) { s1 = warp_sum(s1); s2 = warp_sum(s2); }
-        if (lane == 0) {
-            if (DW == DW_NONE) part[en] = s0;
-            else if (en < P) { part[en] = s0; part[P + en] = s1; part[2 * P + en] = s2; }
-            else part[3 * P + (en - P)] = s0;
-        }
-    }
+// emit functions for mma_tiles_reduce: accumulator index a and tile position pos -> entry of the partial row
+template <int R>
+__device__ __forceinline__ void tp_decode(int tp, int& I, int& J) {
+    constexpr int NB = GramShape<R>::NB;
+    I = 0;
+    while (tp >= NB - I) { tp -= NB - I; I++; }
+    J = I + tp;
 }
 
 template <int R, int DIR, int DOP, int DW>
@@ -194,7 +165,7 @@ k_dir(const DirArgs a) {
     const int nl = R * L, LPZ = (NBUF * nl) | 1;
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                        // [n][LPZ]
-    double* mats = (double*)(z + (size_t)n * LPZ);             // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2
+    double* mats = (double*)(z + dir_zelems(n, LPZ));          // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2
     double2* Et = (double2*)(mats + ((NMAT * RR + 1) & ~1));   // [3][n][L]
     const int tid = threadIdx.x, nth = blockDim.x;
     DirGeom gm;
@@ -260,31 +231,61 @@ k_dir(const DirArgs a) {
     const int pitems = n << lL;                               // tile points (e, l)
 
     if (DOP == DOP_COEFF) {
-        // -------------------------------------------------------------- coefficients (read only)
-        if (a.gram != nullptr) {
-            constexpr int NV = 3 * (R * (R + 1) / 2) + (DW == DW_V ? R : 0);
-            dir_gram<R, DIR, DW, DW == DW_V>(z, LPZ, gm, Et, a.gram + (size_t)blockIdx.x * NV);
+        // -------------------------------------------------------------- coefficients (read only), on the fp64 MMA
+        constexpr int NB = GramShape<R>::NB, NTP = GramShape<R>::NTP;
+        constexpr int P = R * (R + 1) / 2, P2 = R * (R - 1) / 2;
+        constexpr bool WG = (DW != DW_NONE);
+        constexpr int NACCW = WG ? 3 * NTP + (DW == DW_V ? NB : 0) : 1;
+        struct { double acc[3][NTP][2]; double cs[NB][2]; } gw;
+        if (WG && a.gram != nullptr) {
+#pragma unroll
+            for (int d = 0; d < 3; d++)
+#pragma unroll
+                for (int t = 0; t < NTP; t++) gw.acc[d][t][0] = gw.acc[d][t][1] = 0.0;
+#pragma unroll
+            for (int I = 0; I < NB; I++) gw.cs[I][0] = gw.cs[I][1] = 0.0;
+            gram_mma_accum<R, 3, DW == DW_V>(z, LPZ, L, lL, pitems,
+                [&](int e, int l, double2& w0, double2& w1, double2& w2) { dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2); },
+                gw.acc, gw.cs);
             __syncthreads();
         }
         fft_lines_c<false>(z, LPZ, nl, lg, false);
-        constexpr int P2 = R * (R - 1) / 2;
-        const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
-        double* part = a.pgram + (size_t)blockIdx.x * P2;
-        for (int en = warp; en < P2; en += nwarp) {
-            int ca = 0, rem = en;
-            while (rem >= R - 1 - ca) { rem -= R - 1 - ca; ca++; }
-            const int cb = ca + 1 + rem;
-            double s = 0.0;
-            for (int w = lane; w < pitems; w += 32) {
-                const int l = w & (L - 1), e = w >> lL;
-                const double2 za = z[(size_t)e * LPZ + ca * L + l], zb = z[(size_t)e * LPZ + cb * L + l];
-                s = fma(__ldg(a.g.kt2p + e), za.y * zb.x - za.x * zb.y, s);
-            }
-            s = warp_sum(s);
-            if (lane == 0) part[en] = s;
+        double pacc[NTP][2];
+#pragma unroll
+        for (int t = 0; t < NTP; t++) pacc[t][0] = pacc[t][1] = 0.0;
+        parseval_mma_accum<R>(z, LPZ, L, lL, pitems, a.g.kt2p, pacc);
+        __syncthreads();                                        // the tile is free: it becomes the reduction scratch
+        double* scratch = (double*)z;
+        const int cap = 2 * dir_zelems(n, LPZ);
+        if (WG && a.gram != nullptr) {
+            constexpr int NV = 3 * P + (DW == DW_V ? R : 0);
+            double* part = a.gram + (size_t)blockIdx.x * NV;
+            mma_tiles_reduce<NACCW>(&gw.acc[0][0][0], scratch, cap, [&](int ai, int pos, double v) {
+                const int i = pos >> 3, j = pos & 7;
+                if (ai < 3 * NTP) {
+                    const int d = ai / NTP;
+                    int I, J;
+                    tp_decode<R>(ai - d * NTP, I, J);
+                    const int ca = 8 * I + i, cb = 8 * J + j;
+                    if (ca <= cb && cb < R) part[d * P + upper_pair_index(R, ca, cb)] = v;
+                } else {
+                    const int c = 8 * (ai - 3 * NTP) + i;
+                    if (j == 0 && c < R) part[3 * P + c] = v;
+                }
+            });
         }
-        if (a.gram != nullptr) {
-            constexpr int NV = 3 * (R * (R + 1) / 2) + (DW == DW_V ? R : 0);
+        {
+            double* part = a.pgram + (size_t)blockIdx.x * P2;
+            mma_tiles_reduce<NTP>(&pacc[0][0], scratch, cap, [&](int ai, int pos, double v) {
+                const int i = pos >> 3, j = pos & 7;
+                int I, J;
+                tp_decode<R>(ai, I, J);
+                const int ca = 8 * I + i, cb = 8 * J + j;
+                if (ca < cb && cb < R) part[ca * (R - 1) - ca * (ca - 1) / 2 + (cb - ca - 1)] = v;
+            });
+        }
+        if (WG && a.gram != nullptr) {
+            constexpr int NV = 3 * P + (DW == DW_V ? R : 0);
             group_prereduce(a.gram, NV, a.grp_cnt, a.gram2);
         }
         group_prereduce(a.pgram, P2, a.grp_cnt + DLR_CNT_STRIDE, a.pgram2);
@@ -411,8 +412,14 @@ k_dir(const DirArgs a) {
     }
 
     // ------------------------------------------------------------------ sums of the output, store
-    if (a.gram != nullptr)
-        dir_gram<R, DIR, DW_NONE, false>(z, LPZ, gm, Et, a.gram + (size_t)blockIdx.x * (R * (R + 1) / 2));
+    constexpr int NTPo = GramShape<R>::NTP;
+    double gacc[1][NTPo][2];
+    double gcs[GramShape<R>::NB][2];
+    if (a.gram != nullptr) {
+#pragma unroll
+        for (int t = 0; t < NTPo; t++) gacc[0][t][0] = gacc[0][t][1] = 0.0;
+        gram_mma_accum<R, 1, false>(z, LPZ, L, lL, pitems, [](int, int, double2&, double2&, double2&) {}, gacc, gcs);
+    }
     if (a.colsum != nullptr) {
         const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
         for (int c = warp; c < R; c += nwarp) {
@@ -445,7 +452,19 @@ k_dir(const DirArgs a) {
             }
         }
     }
-    if (a.gram != nullptr) group_prereduce(a.gram, R * (R + 1) / 2, a.grp_cnt, a.gram2);
+    if (a.gram != nullptr) {
+        constexpr int P = R * (R + 1) / 2;
+        __syncthreads();                                        // the store has read the tile: it becomes scratch
+        double* part = a.gram + (size_t)blockIdx.x * P;
+        mma_tiles_reduce<NTPo>(&gacc[0][0][0], (double*)z, 2 * dir_zelems(n, LPZ), [&](int ai, int pos, double v) {
+            const int i = pos >> 3, j = pos & 7;
+            int I, J;
+            tp_decode<R>(ai, I, J);
+            const int ca = 8 * I + i, cb = 8 * J + j;
+            if (ca <= cb && cb < R) part[upper_pair_index(R, ca, cb)] = v;
+        });
+        group_prereduce(a.gram, P, a.grp_cnt, a.gram2);
+    }
     if (a.colsum != nullptr) group_prereduce(a.colsum, R, a.grp_cnt + 2 * DLR_CNT_STRIDE, a.colsum2);
 }
 
