@@ -62,6 +62,8 @@ struct dlr_ctx {
     cudaStream_t st, cap_st;
     cudaStream_t side;            // side branch: the coefficient/eigen kernel overlaps the dim-2/3 passes of its transform
     cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_ffork, ev_fjoin;   // field solve on the side stream, joined before the first pass that reads E
+    bool field_pending;
     const RankOps* ops;
     HostGrid gx, gv;
     // big buffers
@@ -463,6 +465,26 @@ void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int 
     CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
 }
 
+// The same solve as a side branch: sub-flows 1 and 2 of the K step that follows do not read E, so the five small
+// kernels of the Poisson solve run beside them; field_join() is called before the first pass that needs E.
+void field_fork(dlr_ctx* c, const double* A, const double* S, const double* vec, int vstride, double scale) {
+    CK(cudaEventRecord(c->ev_ffork, c->st));
+    CK(cudaStreamWaitEvent(c->side, c->ev_ffork, 0));
+    cudaStream_t main_st = c->st;
+    c->st = c->side;
+    field(c, A, S, vec, vstride, scale);
+    c->st = main_st;
+    CK(cudaEventRecord(c->ev_fjoin, c->side));
+    c->count_launches -= 3;
+    c->field_pending = true;
+}
+void field_join(dlr_ctx* c) {
+    if (!c->field_pending) return;
+    CK(cudaStreamWaitEvent(c->st, c->ev_fjoin, 0));
+    c->count_launches -= 1;
+    c->field_pending = false;
+}
+
 // shifted CholeskyQR3 of KL (N x r) -> orthonormal basis (h^3 B^T B = I) into `basis`, coupling matrix into Sout
 // (transS: S = R^T for the L step, Fig. 1 line 40 transpose_inplace).
 // The Gram sums of KL must already be in c->partial, one row per CTA of the pass that produced KL (nblocks0 rows).
@@ -502,7 +524,8 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     // sub-flow 2
     a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
     CK(ops->dir[VD_EXACT2](a, c->st));
-    // sub-flow 3 in the eigenbasis of direction 3
+    // sub-flow 3 in the eigenbasis of direction 3 (the first pass of a K flow that reads the electric field)
+    field_join(c);
     DirArgs e = dirargs(c, hg);
     e.threads = hg.thre; e.L = hg.Le; e.in = c->W; e.E = c->E; e.min_ = mats + 2 * RR; e.Q = c->ft.p.Q;
     e.ez = c->ft.p.ez; e.f1 = c->ft.p.f1; e.f2a = c->ft.p.f2a; e.f2b = c->ft.p.f2b;
@@ -543,7 +566,7 @@ void issue_step(dlr_ctx* c, double tau) {
     //      predictor basis X1 goes to its own buffer: the corrector's first K step starts from X0 again.
     double* Xp = order == 2 ? c->X1 : c->X;
     // ---- line 3: E0 from K0 and V0, eq. (12): rho = -X0 (S0 rho_tilde)
-    field(c, c->X, c->S, c->rho_t, 1, -1.0);
+    field_fork(c, c->X, c->S, c->rho_t, 1, -1.0);
     phase_mark(c, "electric field E0");
     // ---- line 4: K step (Lie, exponential Euler) of length tp with E0;  line 5: QR -> X1, S1
     {
@@ -574,7 +597,7 @@ void issue_step(dlr_ctx* c, double tau) {
     flow(c, gv, c->V, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
     phase_mark(c, "L step (predictor)");
     // ---- Algorithm 2, line 2: E^{1/2} from X1 and L1, eq. (13)
-    field(c, Xp, nullptr, c->zsum, 1, -gv.g.h3);
+    field_fork(c, Xp, nullptr, c->zsum, 1, -gv.g.h3);
     phase_mark(c, "electric field E1/2");
     // ---- line 3: K step (Strang, ETD2RK) of length tau/2 from K0 = X0 S0 with E^{1/2};  line 4: QR -> X2, S3
     {
@@ -679,6 +702,8 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_ffork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fjoin, cudaEventDisableTiming);
     if (e != cudaSuccess) { dlr_destroy(c); return DLR_ERR_CUDA; }
     e = upload_tables(c, c->gx, cfg->x_lo[0], cfg->x_hi[0]);
     if (e == cudaSuccess) e = upload_tables(c, c->gv, cfg->v_lo[0], cfg->v_hi[0]);
@@ -697,6 +722,8 @@ void dlr_destroy(dlr_ctx* c) {
     if (c->side) cudaStreamDestroy(c->side);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->ev_ffork) cudaEventDestroy(c->ev_ffork);
+    if (c->ev_fjoin) cudaEventDestroy(c->ev_fjoin);
     for (auto& p : c->phases) cudaEventDestroy(p.ev);
     delete c;
 }

@@ -8,6 +8,7 @@
 // + split/merge step), so the real data never needs a repacking pass.
 #pragma once
 #include "common.cuh"
+#include "gram_mma.cuh"
 
 enum { D1_IN_REAL = 0, D1_IN_CPLX = 1 };
 enum { D1_OP_NONE = 0, D1_OP_MATVEC = 1, D1_OP_NONLIN_E = 2, D1_OP_NONLIN_V = 3 };
@@ -45,10 +46,16 @@ __host__ __device__ inline int d1_gram_nvals(int R, int kind) {
     return kind == D1_GRAM_PLAIN ? P : kind == D1_GRAM_V ? 3 * P + R : kind == D1_GRAM_E ? 3 * P : 0;
 }
 
+// double2 elements of the tile region: at least the scratch of the cross-warp MMA reduction (64 doubles per warp)
+__host__ __device__ inline int d1_zelems(int M, int LP) {
+    const int need = (DLR_THREADS / 32) * 64 / 2;
+    return M * LP > need ? M * LP : need;
+}
+
 __host__ inline size_t d1_smem_bytes(int n, int RMAX, int T, bool needE, int nmat) {
     const int M = n / 2;
     const int LP = (RMAX * T) | 1;
-    size_t b = (size_t)M * LP * 16 + (size_t)M * 16 + (size_t)nmat * 8;
+    size_t b = (size_t)d1_zelems(M, LP) * 16 + (size_t)M * 16 + (size_t)nmat * 8;
     if (needE) b += (size_t)3 * M * (T | 1) * 16;          // E tile as [d][j][t], t padded to odd
     return b + 16;
 }
@@ -64,7 +71,7 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     const long long q0 = (long long)blockIdx.x * T;          // first row (q = i2 + n*i3)
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                       // [M][LP]
-    double2* tw = z + (size_t)M * LP;                         // [M]  exp(-2 pi i k/n), k < n/2
+    double2* tw = z + d1_zelems(M, LP);                       // [M]  exp(-2 pi i k/n), k < n/2
     double* mat = (double*)(tw + M);                          // [NMAT]
     double2* Et = (double2*)(mat + ((NMAT + 1) & ~1));        // [3][M][TP] (pairs of grid points along i1)
     const int tid = threadIdx.x, nth = blockDim.x;
@@ -192,7 +199,16 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
     }
 
     // ------------------------------------------------------------------ Gram accumulation (ROUT columns)
-    if (GRAM != D1_GRAM_NONE && want_gram) {
+    constexpr int NTPg = GramShape<ROUT>::NTP;
+    double gacc[1][NTPg][2];
+    double gcs[GramShape<ROUT>::NB][2];
+    if (GRAM == D1_GRAM_PLAIN && want_gram) {
+        // plain Gram matrix of the output on the fp64 tensor cores (gram_mma.cuh); reduced across warps after the store
+#pragma unroll
+        for (int t = 0; t < NTPg; t++) gacc[0][t][0] = gacc[0][t][1] = 0.0;
+        gram_mma_accum<ROUT, 1, false>(z, LP, T, lt, M * T, [](int, int, double2&, double2&, double2&) {}, gacc, gcs);
+    }
+    if (GRAM != D1_GRAM_NONE && GRAM != D1_GRAM_PLAIN && want_gram) {
         constexpr int P = ROUT * (ROUT + 1) / 2;
         constexpr int NENT = GRAM == D1_GRAM_V ? P + ROUT : P;      // pairs (+ column sums)
         const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
@@ -272,6 +288,18 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
             row[k] = cadd(ze, wz);
             if (k != M - k) row[M - k] = cconj(csub(ze, wz));
         }
+    }
+    if (GRAM == D1_GRAM_PLAIN && want_gram) {
+        constexpr int P = ROUT * (ROUT + 1) / 2;
+        __syncthreads();                                        // the store has read the tile: it becomes scratch
+        double* part = a.partial + (size_t)blockIdx.x * P;
+        mma_tiles_reduce<NTPg>(&gacc[0][0][0], (double*)z, 2 * d1_zelems(M, LP), [&](int ai, int pos, double v) {
+            constexpr int NB = GramShape<ROUT>::NB;
+            int I = 0, tp = ai;
+            while (tp >= NB - I) { tp -= NB - I; I++; }
+            const int ca = 8 * I + (pos >> 3), cb = 8 * (I + tp) + (pos & 7);
+            if (ca <= cb && cb < ROUT) part[upper_pair_index(ROUT, ca, cb)] = v;
+        });
     }
     if (GRAM != D1_GRAM_NONE && want_gram && a.partial2 != nullptr)
         group_prereduce(a.partial, d1_gram_nvals(ROUT, GRAM), a.grp_cnt, a.partial2);

@@ -116,11 +116,19 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
                     myoff += apq * apq;
                     double c = 1.0, sn = 0.0;
                     if (apq * apq > 1e-40 * nrm2) {
-                        const double theta = (As[cur][q][q] - As[cur][p][p]) / (2.0 * apq);
-                        const double t = fabs(theta) > 1e150 ? 0.5 / theta
-                                                             : copysign(1.0, theta) / (fabs(theta) + sqrt(theta * theta + 1.0));
-                        c = 1.0 / sqrt(t * t + 1.0);
-                        sn = t * c;
+                        // tan of the rotation angle, t = sgn(theta) / (|theta| + sqrt(theta^2 + 1)) with
+                        // theta = (aqq - app) / (2 apq), written so that the dependent chain is two rsqrt and one divide:
+                        // t = 2 apq sgn(d) / (|d| + sqrt(d^2 + 4 apq^2)),  c = 1 / sqrt(1 + t^2),  s = t c
+                        const double d = As[cur][q][q] - As[cur][p][p], x2 = 2.0 * apq;
+                        const double hh = fma(d, d, x2 * x2);
+                        double r = rsqrt(hh);
+                        r = r * fma(-0.5 * hh * r, r, 1.5);            // Newton step: rounding-level 1/sqrt
+                        const double t = copysign(x2, x2 * d) / (fabs(d) + hh * r);
+                        const double tt = fma(t, t, 1.0);
+                        double rc = rsqrt(tt);
+                        rc = rc * fma(-0.5 * tt * rc, rc, 1.5);
+                        c = rc;
+                        sn = t * rc;
                     }
                     alpha[p] = c; beta[p] = -sn; part[p] = q;   // new column p = c a_p - s a_q
                     alpha[q] = c; beta[q] = sn; part[q] = p;    // new column q = s a_p + c a_q
