@@ -50,6 +50,56 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+# kernel families of one step: substring of the launch expression (dlr_set_profiling(ctx, 2)) -> (label, algorithmic
+# bytes per launch as (factor passes, field components): B = 8 N r per factor read or write,
+# 8 N per field component).  Averages over the launches of a step where K and L flows differ.
+FAMILIES = [
+    ("VD_EXACT1", "k_dir<r,1,EXACT> sub-flow 1 + column mixing", 2.0, 0.0),
+    ("VD_EXACT2", "k_dir<r,2,EXACT> sub-flow 2", 2.0, 0.0),
+    ("VD_ETD2", "k_dir<r,3,ETD2> third sub-flow, both ETD2RK stages", 2.0, 2.0),     # E read by 2 of 3 launches
+    ("VD_ETD1", "k_dir<r,3,ETD1> third sub-flow, exponential Euler", 1.5, 1.5),      # K: 2B + E; L (sums only): B
+    ("VD_COEFF1", "k_dir<r,1,COEFF> weighted Gram + Parseval", 1.0, 2.0),
+    ("VD_COEFF2", "k_dir<r,2,COEFF> Parseval", 1.0, 0.0),
+    ("VD_COEFF3", "k_dir<r,3,COEFF> Parseval", 1.0, 0.0),
+    ("V1_APPLY", "k_d1<r,r,MATVEC> CholeskyQR A*R^-1 (+ Gram)", 2.0, 0.0),
+]
+
+
+def kernel_breakdown(ctx, tau, cfg, nprof=5):
+    """per-launch device times of `nprof` steps (CUDA events after every launch, direct launches on the context's
+    stream), grouped into kernel families"""
+    import numpy as np
+    ctx.set_profiling(2)
+    runs = []
+    for _ in range(nprof):
+        ctx.step(tau)
+        runs.append(ctx.phase_times())
+    ctx.set_profiling(0)
+    names = [n for n, _ in runs[0]]
+    ms = np.median(np.array([[t for _, t in r] for r in runs]), axis=0)
+    B = 8.0 * cfg["n_x"] ** 3 * cfg["r"]
+    EN = 8.0 * cfg["n_x"] ** 3
+    fam = {}
+    total = float(sum(t for t in ms if t > 0))
+    for n, t in zip(names, ms):
+        for key, label, nb, ne in FAMILIES:
+            if key in n:
+                if key == "V1_APPLY" and t < 0.010:          # the skipped third CholeskyQR stage: a no-op launch
+                    break
+                f = fam.setdefault(label, {"launches": 0, "ms": 0.0, "bytes": nb * B + ne * EN})
+                f["launches"] += 1
+                f["ms"] += float(t)
+                break
+    out = []
+    for label, f in fam.items():
+        avg_us = 1e3 * f["ms"] / f["launches"]
+        out.append({"kernel": label, "launches_per_step": f["launches"], "avg_us": avg_us,
+                    "share_of_step": f["ms"] / total, "algorithmic_bytes_per_launch": f["bytes"],
+                    "gbs": f["bytes"] / (avg_us * 1e-6) / 1e9})
+    out.sort(key=lambda k: -k["share_of_step"])
+    return out
+
+
 def oracle_leg(cfg, steps, warmup):
     """the oracle as it stands on the host cores, on a bounded sample: `steps` full steps of the SAME workload"""
     import numpy as np
@@ -91,7 +141,7 @@ def main():
     workload = (f"BASELINE.json configs[{args.config - 1}]: {cfg['problem']} {cfg['n_x']}^3x{cfg['n_v']}^3, r={cfg['r']}, "
                 f"tau={cfg['tau']}, Algorithm 2")
     config = {"workload": workload, "n": cfg["n"], "rank": cfg["r"], "tau": cfg["tau"], "parallelism": f"replicas x{args.gpus}",
-              "l2": "working set (~0.3 GB of factors, spectra and work buffers at config 3) exceeds the 126 MB L2; "
+              "l2": "working set (0.14 GB of factors and work buffers at config 3) exceeds the 126 MB L2; "
                     "no explicit flush"}
 
     if args.impl == "reference":
@@ -152,6 +202,7 @@ def main():
     mom = ctx.moments()
     launches = ctx.launches_per_step()
     bytes_step = ctx.bytes_per_step()
+    kernels = kernel_breakdown(ctx, tau, cfg)
 
     # ---- end to end through the public API with HOST buffers: set_initial(host) + K steps + moments() each
     # step (device->host read of the diagnostics) + get_factors(host) at the end, all inside the timed region
@@ -175,6 +226,23 @@ def main():
     if rank == 0:
         peak, peak_src = measured_peak()
         achieved = bytes_step / (ms_step * 1e-3) / 1e9
+        top = kernels[0]
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "r01_traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get(top["kernel"].split(" ")[0])
+        roofline = {
+            "bound": "hbm", "kernel": top["kernel"], "achieved": top["gbs"], "peak": peak, "unit": "GB/s",
+            "frac": top["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": top["algorithmic_bytes_per_launch"], "avg_launch_us": top["avg_us"],
+            "launches_per_step": top["launches_per_step"], "share_of_step": top["share_of_step"],
+            "note": "dominant kernel family of the step by device time; duration = CUDA events after every launch on "
+                    "the context's stream (dlr_set_profiling(ctx, 2), 5 steps, median) right after the timed region; "
+                    "traffic = DRAM bytes per launch from the ncu --set full capture in profiles/ (cold cache)",
+            "step": {"algorithmic_bytes_per_step": bytes_step, "achieved": achieved, "frac": achieved / peak,
+                     "what": "all factor-sized passes of one step (DESIGN.md section 6) / CUDA-event time of the step"},
+            "kernels": kernels,
+        }
         out = {
             "metric": METRIC, "value": ms_step, "unit": "ms/step", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
@@ -186,11 +254,7 @@ def main():
                     "what": f"set_initial(pinned host)+{e2e_steps}x(dlr_step+dlr_moments)+get_factors(host), per step"},
             "gpu_launches": launches * args.steps,
             "launches_per_step": launches,
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src,
-                         "algorithmic_bytes_per_step": bytes_step,
-                         "note": "whole-step figure: algorithmic bytes of the fused byte model (DESIGN.md section 6) / "
-                                 "CUDA-event time of the step; per-kernel figures are in profiles/"},
+            "roofline": roofline,
             "final_state": {"mass": mom["mass"], "electric_energy": mom["electric_energy"],
                             "qr_fallbacks": mom["qr_fallbacks"], "nonfinite": mom["nonfinite"]},
         }

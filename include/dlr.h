@@ -108,7 +108,8 @@ int dlr_get_phase_times(dlr_ctx* ctx, int cap, float* ms, const char** names);
 /* Number of kernel launches one dlr_step issues (for bench.py's gpu_launches). */
 int dlr_launches_per_step(dlr_ctx* ctx);
 
-/* Algorithmic bytes one dlr_step moves under the byte model of DESIGN.md section 6 (for the roofline). */
+/* Algorithmic bytes of the factor-sized passes the last dlr_step issued: every read or
+ * write of an N x r factor counts 8 N r bytes, the field 8 N per component.  0 before the first step. */
 double dlr_bytes_per_step(dlr_ctx* ctx);
 
 /* Kernel-level entry point for tests (all pointers DEVICE, stream of ctx): the batched 3D real-to-complex FFT of

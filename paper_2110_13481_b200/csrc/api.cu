@@ -64,6 +64,7 @@ struct dlr_ctx {
     cudaEvent_t ev_fork, ev_join;
     cudaEvent_t ev_ffork, ev_fjoin;   // field solve on the side stream, joined before the first pass that reads E
     bool field_pending;
+    double bytes_acc, bytes_step;     // algorithmic bytes of the factor-sized passes issued by the current / last step
     const RankOps* ops;
     HostGrid gx, gv;
     // big buffers
@@ -383,6 +384,9 @@ void reduce_partials(dlr_ctx* c, int nblocks, int nvals, double* out2) {
 int d1_blocks(const HostGrid& hg) { return (int)((long long)hg.g.n * hg.g.n / hg.T1); }
 int d3_blocks(const HostGrid& hg) { return (int)(((long long)hg.g.nh * hg.g.n + hg.T3 - 1) / hg.T3); }
 
+// algorithmic bytes: one real factor (N x r doubles) read or written counts B = 8 N r; the field adds 8 N per component
+double fac_bytes(dlr_ctx* c, const HostGrid& hg) { return 8.0 * (double)hg.g.N * c->R; }
+
 DirArgs dirargs(dlr_ctx* c, const HostGrid& hg) {
     DirArgs a;
     memset(&a, 0, sizeof(a));
@@ -401,6 +405,7 @@ void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M
     DirArgs a = dirargs(c, hg);
     a.in = A; a.E = c->E; a.L = hg.Lc; a.gram = c->partial; a.pgram = c->partialP[0]; a.pgram2 = c->pgram2[0]; a.threads = hg.thrc;
     CK(c->ops->dir[kind == 1 ? VD_COEFF1_V : VD_COEFF1_E](a, c->st));
+    c->bytes_acc += 3.0 * fac_bytes(c, hg) + (kind == 2 ? 24.0 * (double)hg.g.N : 0.0);
     // fork: M1 and its eigen-decomposition need only the Gram sums of the pass above; they run beside the two
     // remaining passes (under stream capture this becomes a parallel branch of the step graph)
     CK(cudaEventRecord(c->ev_fork, c->st));
@@ -455,6 +460,7 @@ void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int 
     D1Args a = d1args(c, hg);
     a.in_real = A; a.out_cplx = c->Eh; a.rho_S = S; a.rho_vec = vec; a.rho_stride = vstride; a.rho_scale = scale;
     CK(c->ops->d1[V1_RHO](a, c->st));
+    c->bytes_acc += fac_bytes(c, hg) + 24.0 * (double)hg.g.N;      // read the basis, write E (spectra stay in L2)
     run_d2(c, hg, c->Eh, 1, false);
     D3Args b = d3args(c, hg);
     b.in = c->Eh; b.out = c->Eh; b.T = hg.T3s;
@@ -503,6 +509,7 @@ void qr(dlr_ctx* c, const HostGrid& hg, int nblocks0, double* basis, double* Sou
         D1Args a = d1args(c, hg);
         a.in_real = src[stage]; a.out_real = dst[stage]; a.mat = c->apply; a.partial = c->partial;
         if (stage >= 1) { a.skip_flag = c->status + 1; a.skip_mode = stage; a.out_alt = basis; }
+        if (stage < 2) c->bytes_acc += 2.0 * fac_bytes(c, hg);     // the third stage is skipped in steady state: not counted
         CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
     }
 }
@@ -521,6 +528,7 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     // sub-flow 1:  A <- src (Sin T1), phases, then into the eigenbasis of direction 2
     a.in = src; a.out = c->W; a.min_ = mats + 0 * RR; a.mout = mats + 1 * RR; a.ph = c->ft.p.ph1;
     CK(ops->dir[VD_EXACT1](a, c->st));
+    c->bytes_acc += (order == 1 ? (zero_only ? 5.0 : 6.0) : 10.0) * fac_bytes(c, hg) + (is_L ? 0.0 : 24.0 * (double)hg.g.N);
     // sub-flow 2
     a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
     CK(ops->dir[VD_EXACT2](a, c->st));
@@ -556,6 +564,7 @@ void issue_step(dlr_ctx* c, double tau) {
     double* Sp = order == 2 ? c->Sp : c->S;             // the predictor of Algorithm 2 works on a scratch S
     const PostM2 m2C{&gv, c->C2}, m2D{&gx, c->D2};
     phase_mark(c, "start");
+    c->bytes_acc = 0.0;
     // ---- Algorithm 1, line 1: C coefficients from V0 (kept from the previous step's line 10 when valid)
     if (!c->vh_valid) {
         coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
@@ -592,6 +601,7 @@ void issue_step(dlr_ctx* c, double tau) {
         qr(c, gv, nb, c->V, c->S, 1);                 // line 10: V1, S3 = R^T
         phase_mark(c, "QR L");
         c->vh_valid = false;
+        c->bytes_step = c->bytes_acc;
         return;
     }
     flow(c, gv, c->V, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
@@ -638,6 +648,7 @@ void issue_step(dlr_ctx* c, double tau) {
     qr(c, gx, nb, c->X, c->S, 0);
     phase_mark(c, "QR K (second)");
     c->vh_valid = true;
+    c->bytes_step = c->bytes_acc;
 }
 
 int fail(dlr_ctx* c, cudaError_t e, const char* what) {
@@ -817,11 +828,10 @@ int dlr_run(dlr_ctx* c, double tau, int nsteps) {
 int dlr_launches_per_step(dlr_ctx* c) { return c ? (c->launches ? c->launches : c->count_launches) : 0; }
 
 double dlr_bytes_per_step(dlr_ctx* c) {
-    // byte model of DESIGN.md section 6 (fused design): 110 * B with B = 8 N r per factor;
-    // for N_x != N_v the K-side and L-side shares are weighted 64:46.
-    if (!c) return 0.0;
-    const double Bx = 8.0 * (double)c->gx.g.N * c->R, Bv = 8.0 * (double)c->gv.g.N * c->R;
-    return c->cfg.order == 2 ? 64.0 * Bx + 46.0 * Bv : 24.0 * Bx + 24.0 * Bv;
+    // algorithmic bytes of the factor-sized passes one step issues: every read or write of an
+    // N x r factor counts 8 N r, the field 8 N per component; r x r work and L2-resident single-column spectra are not
+    // counted.  Valid after the first dlr_step.
+    return c ? c->bytes_step : 0.0;
 }
 
 int dlr_set_profiling(dlr_ctx* c, int on) {
