@@ -64,6 +64,7 @@ struct dlr_ctx {
     cudaEvent_t ev_fork, ev_join;
     cudaEvent_t ev_ffork, ev_fjoin;   // field solve on the side stream, joined before the first pass that reads E
     bool field_pending;
+    bool tc_warm, td_warm;            // TC / TD hold a previous eigen-decomposition (warm start of the Jacobi solves)
     double bytes_acc, bytes_step;     // algorithmic bytes of the factor-sized passes issued by the current / last step
     const RankOps* ops;
     HostGrid gx, gv;
@@ -410,8 +411,10 @@ void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M
     // remaining passes (under stream capture this becomes a parallel branch of the step graph)
     CK(cudaEventRecord(c->ev_fork, c->st));
     CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->gram2, dlr_groups(dir_blocks(hg, hg.Lc)), R, kind == 1, hg.g.h3, M1, colsum, T, lam);
+    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->gram2, dlr_groups(dir_blocks(hg, hg.Lc)), R, kind == 1, hg.g.h3, M1, colsum, T, lam,
+                                                     (kind == 1 ? c->tc_warm : c->td_warm) ? 1 : 0);
     CK(cudaGetLastError());
+    (kind == 1 ? c->tc_warm : c->td_warm) = true;
     CK(cudaEventRecord(c->ev_join, c->side));
     c->count_launches -= 3;                         // the three event calls above are not kernel launches
     a.gram = nullptr; a.E = nullptr;
@@ -771,6 +774,7 @@ int dlr_set_initial(dlr_ctx* c, const double* X, const double* S, const double* 
     if (e != cudaSuccess) return fail(c, e, "dlr_set_initial copy");
     c->vh_valid = false;
     c->has_state = false;
+    c->tc_warm = c->td_warm = false;
     int rc = gram_check(c, c->gx, c->X);
     if (rc == DLR_OK) rc = gram_check(c, c->gv, c->V);
     if (rc != DLR_OK) return rc;

@@ -69,7 +69,7 @@ __device__ __forceinline__ void cta_reduce_rows(const double* __restrict__ parti
 #define DLR_EIG_THREADS 256
 __global__ void __launch_bounds__(DLR_EIG_THREADS)
 k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double h3, double* M1, double* colsum,
-             double* Tout, double* lam) {
+             double* Tout, double* lam, int warm) {
     __shared__ double As[2][DLR_RMAXS][DLR_RMAXS + 1], Ts[2][DLR_RMAXS][DLR_RMAXS + 1];
     __shared__ double red[DLR_RMAXS * (DLR_RMAXS + 1) / 2], tmp[DLR_EIG_THREADS];
     __shared__ double alpha[DLR_RMAXS], beta[DLR_RMAXS], sq[DLR_RMAXS];
@@ -92,6 +92,30 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
         M1[(size_t)d * RR + idx] = v;
     }
     __syncthreads();
+    if (warm) {
+        // warm start: the matrix changes little between consecutive solves, so the previous eigenvectors Tp (still in
+        // Tout) almost diagonalise it: iterate on Tp^T A Tp and accumulate the rotations onto Tp (2-3 sweeps instead
+        // of ~8).  T diag(lam) T^T is gauge-free, so the result is as valid as a cold start.
+        for (int idx = tid; idx < RR; idx += nth) Ts[0][idx / R][idx % R] = Tout[(size_t)d * RR + idx];
+        __syncthreads();
+        for (int idx = tid; idx < RR; idx += nth) {            // B = A Tp
+            const int i = idx / R, j = idx - i * R;
+            double acc = 0.0;
+            for (int k = 0; k < R; k++) acc = fma(As[0][i][k], Ts[0][k][j], acc);
+            As[1][i][j] = acc;
+        }
+        __syncthreads();
+        for (int idx = tid; idx < RR; idx += nth) {            // A' = Tp^T B, upper part mirrored
+            const int i = idx / R, j = idx - i * R;
+            if (i <= j) {
+                double acc = 0.0;
+                for (int k = 0; k < R; k++) acc = fma(Ts[0][k][i], As[1][k][j], acc);
+                As[0][i][j] = acc;
+                As[0][j][i] = acc;
+            }
+        }
+        __syncthreads();
+    }
     if (tid < 32) {
         double nr = 0.0;
         for (int idx = tid; idx < RR; idx += 32) { const double v = As[0][idx / R][idx % R]; nr += v * v; }
@@ -157,6 +181,31 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
         }
         __syncthreads();
         if (s_off2 <= 1e-32 * nrm2) break;                     // off-diagonal norm met in this sweep <= 1e-16 ||A||_F
+    }
+    if (warm) {
+        // one Newton-Schulz step T <- T (3 I - T^T T) / 2 keeps the accumulated T orthogonal to rounding level no matter
+        // how many steps it has been carried along
+        const int oth = cur ^ 1;
+        for (int idx = tid; idx < RR; idx += nth) {            // G = T^T T
+            const int i = idx / R, j = idx - i * R;
+            double acc = 0.0;
+            for (int k = 0; k < R; k++) acc = fma(Ts[cur][k][i], Ts[cur][k][j], acc);
+            Ts[oth][i][j] = acc;
+        }
+        __syncthreads();
+        for (int idx = tid; idx < RR; idx += nth) {            // T (1.5 I - 0.5 G), into the free half of As
+            const int i = idx / R, j = idx - i * R;
+            double acc = 0.0;
+            for (int k = 0; k < R; k++) acc = fma(Ts[cur][i][k], Ts[oth][k][j], acc);
+            As[oth][i][j] = 1.5 * Ts[cur][i][j] - 0.5 * acc;
+        }
+        __syncthreads();
+        for (int idx = tid; idx < RR; idx += nth) {
+            const int i = idx / R, j = idx - i * R;
+            Tout[(size_t)d * RR + idx] = As[oth][i][j];
+            if (i == j) lam[d * R + i] = As[cur][i][i];
+        }
+        return;
     }
     for (int idx = tid; idx < RR; idx += nth) {
         const int i = idx / R, j = idx - i * R;
