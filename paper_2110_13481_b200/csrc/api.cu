@@ -113,7 +113,7 @@ int choose_T1(int n, int RMAX, bool needE, int nmat) {
     for (int T = 1; T <= rows && T <= 64; T *= 2) {
         const size_t sm = d1_smem_bytes(n, RMAX, T, needE, nmat);
         if (sm > SMEM_TARGET && T > 1) break;
-        if (rows / T >= 296 || T <= 4) best = T;
+        if (rows / T >= 148 || T <= 4) best = T;     // measured: larger tiles win as long as every SM gets one
     }
     while (best > 1 && d1_smem_bytes(n, RMAX, best, needE, nmat) > SMEM_MAX) best /= 2;
     return best;
@@ -286,9 +286,9 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     hg.thre = dthreads(tune("thre", DLR_THREADS));
     hg.thrc = dthreads(tune("thrc", DLR_THREADS));
     const int lmax = 8;
-    hg.Lx = choose_L(n, R, 1, 2, false, (size_t)tune("smx", 48) * 1024, lmax);
+    hg.Lx = choose_L(n, R, 1, 2, false, (size_t)tune("smx", 96) * 1024, lmax);
     hg.Le = choose_L(n, R, 2, 5, true, (size_t)tune("sme", 110) * 1024, lmax);
-    hg.Lc = choose_L(n, R, 1, 2, true, (size_t)tune("smc", 64) * 1024, lmax);
+    hg.Lc = choose_L(n, R, 1, 2, true, (size_t)tune("smc", 110) * 1024, lmax);
     const int lx = tune("lx", 0), le = tune("le", 0), lc = tune("lc", 0);
     if (is_pow2(lx) && lx <= n / 2 && dir_smem_bytes(n, R, lx, 1, 2, false) <= SMEM_MAX) hg.Lx = lx;
     if (is_pow2(le) && le <= n / 2 && dir_smem_bytes(n, R, le, 2, 5, true) <= SMEM_MAX) hg.Le = le;

@@ -122,6 +122,23 @@ __device__ __forceinline__ void dir_matvec(double2 (&x)[R], const double* A) {  
     for (int c = 0; c < R; c++) x[c] = y[c];
 }
 
+// out[co * stride] = (x A)[co], streamed out one component at a time (x is fully in registers, so out may alias the
+// place x was loaded from): no second r-vector in registers
+template <int R>
+__device__ __forceinline__ void dir_matvec_store(const double2 (&x)[R], const double* A, double2* out, int stride) {
+#pragma unroll
+    for (int co = 0; co < R; co++) {
+        double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int ci = 0; ci < R; ci++) {
+            const double m = A[ci * R + co];
+            acc.x = fma(m, x[ci].x, acc.x);
+            acc.y = fma(m, x[ci].y, acc.y);
+        }
+        out[co * stride] = acc;
+    }
+}
+
 // real-space term in the eigenbasis: g = sum_i w_i o (m Q_i), component co written to gout[co * stride]
 // (streamed out one component at a time: only m stays in registers)
 template <int R>
@@ -302,9 +319,7 @@ k_dir(const DirArgs a) {
                 double2 x[R];
 #pragma unroll
                 for (int c = 0; c < R; c++) x[c] = p[c * L];
-                dir_matvec<R>(x, mats);
-#pragma unroll
-                for (int c = 0; c < R; c++) p[c * L] = x[c];
+                dir_matvec_store<R>(x, mats, p, L);
             }
             __syncthreads();
         }
@@ -325,9 +340,7 @@ k_dir(const DirArgs a) {
                 double2 x[R];
 #pragma unroll
                 for (int c = 0; c < R; c++) x[c] = p[c * L];
-                dir_matvec<R>(x, mats + RR);
-#pragma unroll
-                for (int c = 0; c < R; c++) p[c * L] = x[c];
+                dir_matvec_store<R>(x, mats + RR, p, L);
             }
             __syncthreads();
         }
