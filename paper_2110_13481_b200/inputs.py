@@ -63,7 +63,7 @@ def _band_limited_columns(rng, n, ncols, band):
         co = rng.standard_normal((nb, nb, band + 1)) + 1j * rng.standard_normal((nb, nb, band + 1))
         idx = np.r_[0:band + 1, n - band:n]
         spec[np.ix_(idx, idx, np.arange(band + 1))] = co
-        cols[:, c] = np.fft.irfftn(spec, s=(n, n, n)).reshape(-1)
+        cols[:, c] = np.fft.irfftn(spec, s=(n, n, n), axes=(0, 1, 2)).reshape(-1)
     return cols
 
 
