@@ -162,3 +162,46 @@ __device__ __forceinline__ void fft_mid(double2* s, int LP, int nlines, int logM
     }
     __syncthreads();
 }
+
+// Two-buffer variant of fft_mid for the exponential Runge-Kutta passes: lines `line` of buffer A (s) and of buffer B
+// (s + boff) are processed together.  FA / FB: run the last forward group on A / B first (otherwise the data already
+// is in that state);  f(a, b, stored position e, line) combines the two spectra element by element;  IA / IB: run
+// the first inverse group on A / B afterwards;  SA / SB: store A / B back.
+template <int G, bool FA, bool FB, bool IA, bool IB, bool SA, bool SB, class F>
+__device__ __forceinline__ void fft_mid2_group(double2* s, int boff, int LP, FastDiv nl, int logM, F f) {
+    constexpr int R = 1 << G;
+    const int nlines = (int)nl.d;
+    const int items = (1 << (logM - G)) * nlines;
+    for (int w = threadIdx.x; w < items; w += blockDim.x) {
+        const int b = (int)fdiv((unsigned)w, nl);
+        const int line = w - b * nlines;
+        double2* p = s + (size_t)(b << G) * LP + line;
+        double2 a[R], bb[R];
+#pragma unroll
+        for (int q = 0; q < R; q++) { a[q] = p[(size_t)q * LP]; bb[q] = p[(size_t)q * LP + boff]; }
+        if (FA) bfly<G, false>(a);
+        if (FB) bfly<G, false>(bb);
+#pragma unroll
+        for (int q = 0; q < R; q++) f(a[q], bb[q], (b << G) + q, line);
+        if (IA) bfly<G, true>(a);
+        if (IB) bfly<G, true>(bb);
+#pragma unroll
+        for (int q = 0; q < R; q++) {
+            if (SA) p[(size_t)q * LP] = a[q];
+            if (SB) p[(size_t)q * LP + boff] = bb[q];
+        }
+    }
+}
+
+template <bool FA, bool FB, bool IA, bool IB, bool SA, bool SB, class F>
+__device__ __forceinline__ void fft_mid2(double2* s, int boff, int LP, int nlines, int logM, F f) {
+    int g[3], ng;
+    fft_plan(logM, g, ng);
+    const FastDiv nl = make_fastdiv((unsigned)nlines);
+    switch (g[ng - 1]) {
+        case 1: fft_mid2_group<1, FA, FB, IA, IB, SA, SB>(s, boff, LP, nl, logM, f); break;
+        case 2: fft_mid2_group<2, FA, FB, IA, IB, SA, SB>(s, boff, LP, nl, logM, f); break;
+        default: fft_mid2_group<3, FA, FB, IA, IB, SA, SB>(s, boff, LP, nl, logM, f); break;
+    }
+    __syncthreads();
+}

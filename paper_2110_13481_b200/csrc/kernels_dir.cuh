@@ -365,28 +365,25 @@ k_dir(const DirArgs a) {
             dir_nonlin<R>(x, p + nl, L, Q, w0, w1, w2);
         }
         __syncthreads();
-        fft_lines_c<false>(z, LPZ, 2 * nl, lg, false);
-        {
-            const int items = nl << lg;
-            const FastDiv fnl = make_fastdiv((unsigned)nl);
-            for (int w = tid; w < items; w += nth) {
-                const int e = (int)fdiv((unsigned)w, fnl), line = w - e * nl;
+        // Fourier-space stages fused into the middle FFT group (fft_mid2): the spectra of m and g0 never make a round
+        // trip through shared memory.  a = e^z M^ + t phi1 G0^  (stage-1 state);  ETD2RK keeps  e^z M^ + t (phi1 - phi2) G0^
+        // in buffer A (spectral) and adds t phi2 G1^ to it after the second evaluation of the real-space term.
+        fft_lines_c<false>(z, LPZ, 2 * nl, lg, true);
+        if (DOP == DOP_ETD1) {
+            fft_mid2<true, true, true, false, true, false>(z, nl, LPZ, nl, lg, [&](double2& av, double2& bv, int e, int line) {
                 const int c = line >> lL;
-                double2* p = z + (size_t)e * LPZ + line;
-                const double2 Mh = p[0], Gh = p[nl];
-                const double2 em = cmul(Mh, __ldg(a.ez + (size_t)e * R + c));
-                const double2 ah = cadd(em, cmul(Gh, __ldg(a.f1 + (size_t)e * R + c)));
-                if (DOP == DOP_ETD1) {
-                    p[0] = ah;
-                } else {
-                    p[nl] = ah;                               // a^ (stage-1 state), inverse-transformed for N'(a)
-                    p[0] = cadd(em, cmul(Gh, __ldg(a.f2a + (size_t)e * R + c)));
-                }
-            }
-        }
-        __syncthreads();
-        if (DOP == DOP_ETD2) {
-            fft_lines_c<true>(z + nl, LPZ, nl, lg, false);
+                av = cadd(cmul(av, __ldg(a.ez + (size_t)e * R + c)), cmul(bv, __ldg(a.f1 + (size_t)e * R + c)));
+            });
+            fft_lines_c<true>(z, LPZ, nl, lg, true);
+        } else {
+            fft_mid2<true, true, false, true, true, true>(z, nl, LPZ, nl, lg, [&](double2& av, double2& bv, int e, int line) {
+                const int c = line >> lL;
+                const double2 em = cmul(av, __ldg(a.ez + (size_t)e * R + c));
+                const double2 ah = cadd(em, cmul(bv, __ldg(a.f1 + (size_t)e * R + c)));
+                av = cadd(em, cmul(bv, __ldg(a.f2a + (size_t)e * R + c)));
+                bv = ah;                                      // inverse-transformed for N'(a)
+            });
+            fft_lines_c<true>(z + nl, LPZ, nl, lg, true);
             for (int w = tid; w < pitems; w += nth) {         // g1 = N'(a)
                 const int l = w & (L - 1), e = w >> lL;
                 double2* p = z + (size_t)e * LPZ + nl + l;
@@ -398,20 +395,12 @@ k_dir(const DirArgs a) {
                 dir_nonlin<R>(x, p, L, Q, w0, w1, w2);            // x is fully in registers: in-place is safe
             }
             __syncthreads();
-            fft_lines_c<false>(z + nl, LPZ, nl, lg, false);
-            {
-                const int items = nl << lg;
-                const FastDiv fnl = make_fastdiv((unsigned)nl);
-                for (int w = tid; w < items; w += nth) {
-                    const int e = (int)fdiv((unsigned)w, fnl), line = w - e * nl;
-                    const int c = line >> lL;
-                    double2* p = z + (size_t)e * LPZ + line;
-                    p[0] = cadd(p[0], cmul(p[nl], __ldg(a.f2b + (size_t)e * R + c)));
-                }
-            }
-            __syncthreads();
+            fft_lines_c<false>(z + nl, LPZ, nl, lg, true);
+            fft_mid2<false, true, true, false, true, false>(z, nl, LPZ, nl, lg, [&](double2& av, double2& bv, int e, int line) {
+                av = cadd(av, cmul(bv, __ldg(a.f2b + (size_t)e * R + (line >> lL))));
+            });
+            fft_lines_c<true>(z, LPZ, nl, lg, true);
         }
-        fft_lines_c<true>(z, LPZ, nl, lg, false);
         for (int w = tid; w < pitems; w += nth) {             // scale of the inverse transform, back to the output basis
             const int l = w & (L - 1), e = w >> lL;
             double2* p = z + (size_t)e * LPZ + l;
