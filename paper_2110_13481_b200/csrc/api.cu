@@ -43,6 +43,7 @@ struct HostGrid {
     int thr1, thr2, thr3; // CTA sizes of the three pass families
     int Lx, Le, Lc;       // directional passes: packed lines per column for EXACT, ETD and COEFF tiles
     int thrx, thre, thrc; // CTA sizes of the EXACT, ETD and COEFF directional passes
+    int thrx2;            // CTA size of the direction-2 sub-flow (register-light: up to 512 threads)
 };
 
 struct FlowTab {
@@ -284,15 +285,28 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     auto dthreads = [](int t) { return (t >= 64 && t <= DLR_THREADS && t % 32 == 0) ? t : DLR_THREADS; };
     hg.thrx = dthreads(tune("thrx", DLR_THREADS));
     hg.thre = dthreads(tune("thre", DLR_THREADS));
+    { const int t = tune("thrx2", 0); hg.thrx2 = (t >= 64 && t <= 2 * DLR_THREADS && t % 32 == 0) ? t : 0; }
     hg.thrc = dthreads(tune("thrc", DLR_THREADS));
     const int lmax = 8;
     hg.Lx = choose_L(n, R, 1, 2, false, (size_t)tune("smx", 96) * 1024, lmax);
     hg.Le = choose_L(n, R, 2, 5, true, (size_t)tune("sme", 110) * 1024, lmax);
     hg.Lc = choose_L(n, R, 1, 2, true, (size_t)tune("smc", 110) * 1024, lmax);
+    // a tile with a single packed line per column means 16-byte strided segments in directions 2 and 3: measured at
+    // configs 4 and 5 it pays to give such a tile all of the shared memory (one CTA per SM) to reach two lines
+    const size_t smem_all = SMEM_MAX - 1024;
+    if (hg.Lx < 2) hg.Lx = choose_L(n, R, 1, 2, false, smem_all, 2);
+    if (hg.Le < 2) hg.Le = choose_L(n, R, 2, 5, true, smem_all, 2);
+    if (hg.Lc < 2) hg.Lc = choose_L(n, R, 1, 2, true, smem_all, 2);
     const int lx = tune("lx", 0), le = tune("le", 0), lc = tune("lc", 0);
     if (is_pow2(lx) && lx <= n / 2 && dir_smem_bytes(n, R, lx, 1, 2, false) <= SMEM_MAX) hg.Lx = lx;
     if (is_pow2(le) && le <= n / 2 && dir_smem_bytes(n, R, le, 2, 5, true) <= SMEM_MAX) hg.Le = le;
     if (is_pow2(lc) && lc <= n / 2 && dir_smem_bytes(n, R, lc, 1, 2, true) <= SMEM_MAX) hg.Lc = lc;
+    if (hg.thrx2 == 0) {
+        // the direction-2 sub-flow is register-light (up to 512 threads per CTA): 320 threads when the butterfly items of
+        // an FFT group (n/8 per line) then divide evenly, e.g. 640 items at n = 64, r = 10, 8 lines per column
+        const int items = (n / 8) * R * hg.Lx;
+        hg.thrx2 = (n >= 8 && items % 320 == 0) ? 320 : DLR_THREADS;
+    }
 }
 
 cudaError_t upload_tables(dlr_ctx* c, HostGrid& hg, double lo, double hi) {
@@ -533,8 +547,9 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     CK(ops->dir[VD_EXACT1](a, c->st));
     c->bytes_acc += (order == 1 ? (zero_only ? 5.0 : 6.0) : 10.0) * fac_bytes(c, hg) + (is_L ? 0.0 : 24.0 * (double)hg.g.N);
     // sub-flow 2
-    a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
+    a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2; a.threads = hg.thrx2;
     CK(ops->dir[VD_EXACT2](a, c->st));
+    a.threads = hg.thrx;
     // sub-flow 3 in the eigenbasis of direction 3 (the first pass of a K flow that reads the electric field)
     field_join(c);
     DirArgs e = dirargs(c, hg);
@@ -553,7 +568,9 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     }
     e.mout = mats + 5 * RR; e.store = 1; e.out = c->W;          // T3^T T2
     CK(ops->dir[is_L ? VD_ETD2_V : VD_ETD2_E](e, c->st));
+    a.threads = hg.thrx2;
     CK(ops->dir[VD_EXACT2](a, c->st));                           // sub-flow 2, second half
+    a.threads = hg.thrx;
     a.out = c->KL; a.min_ = mats + 6 * RR; a.mout = mats + 7 * RR; a.ph = c->ft.p.ph1; a.gram = c->partial;
     CK(ops->dir[VD_EXACT1](a, c->st));                           // sub-flow 1, second half, + Gram of the result
     return dir_blocks(hg, hg.Lx);
