@@ -387,7 +387,6 @@ D3Args d3args(dlr_ctx* c, const HostGrid& hg) {
     D3Args a;
     memset(&a, 0, sizeof(a));
     a.g = hg.g; a.T = hg.T3; a.e_scale = c->cfg.e_scale; a.threads = hg.thr3;
-    a.mats = c->ft.p.mats; a.ph1 = c->ft.p.ph1; a.ph2 = c->ft.p.ph2; a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1;
     return a;
 }
 

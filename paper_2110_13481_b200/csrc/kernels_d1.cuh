@@ -1,18 +1,18 @@
-// Dimension-1 pass: everything that happens while a tile of grid rows (lines along i1) of ALL columns sits in
-// shared memory in real space:
-//   load (real rows, or half-spectrum rows + complex-to-real inverse transform along dim 1)
-//   -> point-wise operation across the columns (K = A*Mat; the non-diagonal terms of eqs. (9)/(11))
-//   -> weighted Gram accumulation (C1/D1 of PAPER.md:150,162; rho_tilde of eq. (12); Gram matrix for CholeskyQR)
-//   -> store (real rows and/or real-to-complex forward transform along dim 1 into the half spectrum).
+// Row-tile pass: a tile of grid rows (lines along i1) of ALL columns sits in shared memory in real space.  Used for
+//   * the A*R^-1 passes of CholeskyQR (real in -> A*Mat -> Gram of the result on the fp64 tensor cores -> real out),
+//   * the Gram check of dlr_set_initial,
+//   * the first and last pass of the single-column 3D FFT of the Poisson solve: rho = A p followed by the real-to-complex
+//     transform along dim 1 into the half spectrum, and the complex-to-real inverse of the three field components.
 // A real row of n doubles is handled as n/2 complex numbers z[j] = a[2j] + i a[2j+1] (half-length complex FFT
 // + split/merge step), so the real data never needs a repacking pass.
+// (The K/L flows and the coefficient sums use the directional passes of kernels_dir.cuh.)
 #pragma once
 #include "common.cuh"
 #include "gram_mma.cuh"
 
 enum { D1_IN_REAL = 0, D1_IN_CPLX = 1 };
-enum { D1_OP_NONE = 0, D1_OP_MATVEC = 1, D1_OP_NONLIN_E = 2, D1_OP_NONLIN_V = 3 };
-enum { D1_GRAM_NONE = 0, D1_GRAM_PLAIN = 1, D1_GRAM_V = 2, D1_GRAM_E = 3 };
+enum { D1_OP_NONE = 0, D1_OP_MATVEC = 1 };
+enum { D1_GRAM_NONE = 0, D1_GRAM_PLAIN = 1 };
 enum { D1_OUT_NONE = 0, D1_OUT_REAL = 1, D1_OUT_CPLX = 2, D1_OUT_BOTH = 3 };
 
 struct D1Args {
@@ -21,8 +21,7 @@ struct D1Args {
     const double2* in_cplx;    // RIN columns, stride NC
     double* out_real;          // ROUT columns
     double2* out_cplx;         // ROUT columns
-    const double* mat;         // MATVEC: [RIN][ROUT];  NONLIN: 3 x [R][R], out_c = sum_i w_i sum_c' M_i[c][c'] a_c'
-    const double* E;           // [3][N] weights for NONLIN_E / GRAM_E
+    const double* mat;         // MATVEC: [RIN][ROUT]
     double* partial;           // [gridDim.x][nvals] Gram partial sums
     double* partial2;          // [groups][nvals] group sums (see group_prereduce), or nullptr
     unsigned* grp_cnt;         // group counters
@@ -43,7 +42,7 @@ struct D1Args {
 
 __host__ __device__ inline int d1_gram_nvals(int R, int kind) {
     const int P = R * (R + 1) / 2;
-    return kind == D1_GRAM_PLAIN ? P : kind == D1_GRAM_V ? 3 * P + R : kind == D1_GRAM_E ? 3 * P : 0;
+    return kind == D1_GRAM_PLAIN ? P : 0;
 }
 
 // double2 elements of the tile region: at least the scratch of the cross-warp MMA reduction (64 doubles per warp)
@@ -56,24 +55,22 @@ __host__ inline size_t d1_smem_bytes(int n, int RMAX, int T, bool needE, int nma
     const int M = n / 2;
     const int LP = (RMAX * T) | 1;
     size_t b = (size_t)d1_zelems(M, LP) * 16 + (size_t)M * 16 + (size_t)nmat * 8;
-    if (needE) b += (size_t)3 * M * (T | 1) * 16;          // E tile as [d][j][t], t padded to odd
+    (void)needE;
     return b + 16;
 }
 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
 __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 ? 2 : 1)) k_d1(const D1Args a) {
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
-    constexpr bool NEED_E = (OP == D1_OP_NONLIN_E) || (GRAM == D1_GRAM_E);
-    constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : (OP == D1_OP_NONLIN_E || OP == D1_OP_NONLIN_V) ? 3 * RIN * RIN : 0;
+    constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : 0;
     const int n = a.g.n, M = n >> 1, lg = a.g.log2n, logM = lg - 1, T = a.T;
-    const int lt = __ffs(T) - 1, TP = T | 1;                  // log2(T); padded t-stride of the E tile
+    const int lt = __ffs(T) - 1;                              // log2(T)
     const int nlines = RMAX * T, LP = nlines | 1;
     const long long q0 = (long long)blockIdx.x * T;          // first row (q = i2 + n*i3)
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                       // [M][LP]
     double2* tw = z + d1_zelems(M, LP);                       // [M]  exp(-2 pi i k/n), k < n/2
     double* mat = (double*)(tw + M);                          // [NMAT]
-    double2* Et = (double2*)(mat + ((NMAT + 1) & ~1));        // [3][M][TP] (pairs of grid points along i1)
     const int tid = threadIdx.x, nth = blockDim.x;
     double* out_real = a.out_real;
     bool want_gram = true;
@@ -94,16 +91,6 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
         }
     } else {
         for (int i = tid; i < NMAT; i += nth) mat[i] = a.mat[i];
-    }
-    if (NEED_E) {
-        const int cnt = T * M;                                // double2 per component
-        for (int d = 0; d < 3; d++) {
-            const double2* src = (const double2*)(a.E + (size_t)d * a.g.N) + q0 * M;
-            for (int i = tid; i < cnt; i += nth) {
-                const int t = i >> logM, j = i & (M - 1);
-                Et[(size_t)(d * M + j) * TP + t] = src[i];
-            }
-        }
     }
     if (IN_MODE == D1_IN_CPLX) __syncthreads();               // tw needed by the merge step below
 
@@ -166,33 +153,6 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
                     }
                     p[co * T] = acc;
                 }
-            } else {
-                double2 w0, w1, w2;
-                if (OP == D1_OP_NONLIN_E) {
-                    w0 = Et[(size_t)(0 * M + j) * TP + t];
-                    w1 = Et[(size_t)(1 * M + j) * TP + t];
-                    w2 = Et[(size_t)(2 * M + j) * TP + t];
-                } else {
-                    const int q = (int)q0 + t;
-                    const int i2 = q & (n - 1), i3 = q >> lg;
-                    w0 = make_double2(a.g.lo + a.g.h * (2 * j), a.g.lo + a.g.h * (2 * j + 1));
-                    w1 = make_double2(a.g.lo + a.g.h * i2, a.g.lo + a.g.h * i2);
-                    w2 = make_double2(a.g.lo + a.g.h * i3, a.g.lo + a.g.h * i3);
-                }
-#pragma unroll
-                for (int co = 0; co < ROUT; co++) {
-                    double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
-#pragma unroll
-                    for (int ci = 0; ci < RIN; ci++) {
-                        const double m0 = mat[co * RIN + ci], m1 = mat[RIN * RIN + co * RIN + ci],
-                                     m2 = mat[2 * RIN * RIN + co * RIN + ci];
-                        s0.x = fma(m0, x[ci].x, s0.x); s0.y = fma(m0, x[ci].y, s0.y);
-                        s1.x = fma(m1, x[ci].x, s1.x); s1.y = fma(m1, x[ci].y, s1.y);
-                        s2.x = fma(m2, x[ci].x, s2.x); s2.y = fma(m2, x[ci].y, s2.y);
-                    }
-                    p[co * T] = make_double2(fma(w0.x, s0.x, fma(w1.x, s1.x, w2.x * s2.x)),
-                                             fma(w0.y, s0.y, fma(w1.y, s1.y, w2.y * s2.y)));
-                }
             }
         }
         __syncthreads();
@@ -207,55 +167,6 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
 #pragma unroll
         for (int t = 0; t < NTPg; t++) gacc[0][t][0] = gacc[0][t][1] = 0.0;
         gram_mma_accum<ROUT, 1, false>(z, LP, T, lt, M * T, [](int, int, double2&, double2&, double2&) {}, gacc, gcs);
-    }
-    if (GRAM != D1_GRAM_NONE && GRAM != D1_GRAM_PLAIN && want_gram) {
-        constexpr int P = ROUT * (ROUT + 1) / 2;
-        constexpr int NENT = GRAM == D1_GRAM_V ? P + ROUT : P;      // pairs (+ column sums)
-        const int warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
-        const int items = M * T;
-        double* part = a.partial + (size_t)blockIdx.x * d1_gram_nvals(ROUT, GRAM);
-        for (int e = warp; e < NENT; e += nwarp) {
-            int ca = 0, cb = 0;
-            if (e < P) {                                            // decode pair index -> (ca <= cb)
-                int rem = e;
-                while (rem >= ROUT - ca) { rem -= ROUT - ca; ca++; }
-                cb = ca + rem;
-            } else {
-                ca = cb = e - P;
-            }
-            double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-            for (int w = lane; w < items; w += 32) {
-                const int t = w & (T - 1), j = w >> lt;
-                const double2 za = z[(size_t)j * LP + ca * T + t];
-                if (e >= P) { s0 += za.x + za.y; continue; }
-                const double2 zb = z[(size_t)j * LP + cb * T + t];
-                const double px = za.x * zb.x, py = za.y * zb.y;
-                if (GRAM == D1_GRAM_PLAIN) {
-                    s0 += px + py;
-                } else if (GRAM == D1_GRAM_E) {
-                    const double2 w0 = Et[(size_t)(0 * M + j) * TP + t];
-                    const double2 w1 = Et[(size_t)(1 * M + j) * TP + t];
-                    const double2 w2 = Et[(size_t)(2 * M + j) * TP + t];
-                    s0 = fma(w0.x, px, fma(w0.y, py, s0));
-                    s1 = fma(w1.x, px, fma(w1.y, py, s1));
-                    s2 = fma(w2.x, px, fma(w2.y, py, s2));
-                } else {
-                    const int q = (int)q0 + t;
-                    const int i2 = q & (n - 1), i3 = q >> lg;
-                    const double v1a = a.g.lo + a.g.h * (2 * j), v1b = a.g.lo + a.g.h * (2 * j + 1);
-                    s0 = fma(v1a, px, fma(v1b, py, s0));
-                    s1 = fma(a.g.lo + a.g.h * i2, px + py, s1);
-                    s2 = fma(a.g.lo + a.g.h * i3, px + py, s2);
-                }
-            }
-            s0 = warp_sum(s0);
-            if (GRAM == D1_GRAM_V || GRAM == D1_GRAM_E) { s1 = warp_sum(s1); s2 = warp_sum(s2); }
-            if (lane == 0) {
-                if (GRAM == D1_GRAM_PLAIN) part[e] = s0;
-                else if (e < P) { part[e] = s0; part[P + e] = s1; part[2 * P + e] = s2; }
-                else part[3 * P + (e - P)] = s0;
-            }
-        }
     }
 
     // ------------------------------------------------------------------ store
@@ -308,10 +219,9 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
 inline cudaError_t launch_d1(const D1Args& a, cudaStream_t st) {
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
-    constexpr bool NEED_E = (OP == D1_OP_NONLIN_E) || (GRAM == D1_GRAM_E);
-    constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : (OP == D1_OP_NONLIN_E || OP == D1_OP_NONLIN_V) ? 3 * RIN * RIN : 0;
+    constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : 0;
     auto kern = k_d1<RIN, ROUT, IN_MODE, OP, GRAM, OUT_MODE>;
-    const size_t sm = d1_smem_bytes(a.g.n, RMAX, a.T, NEED_E, (NMAT + 1) & ~1);
+    const size_t sm = d1_smem_bytes(a.g.n, RMAX, a.T, false, (NMAT + 1) & ~1);
     static size_t configured = 0;
     if (sm > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);

@@ -23,12 +23,6 @@ __global__ void k_reduce_partials(const double* __restrict__ partial, int nblock
     }
 }
 
-__device__ __forceinline__ double sum_g1(const double* p2, int nvals, int v) {
-    double s = 0.0;
-    for (int g = 0; g < DLR_G1; g++) s += p2[(size_t)g * nvals + v];
-    return s;
-}
-
 // CTA-wide deterministic reduction of per-CTA partial rows, done by the consumer kernel itself (no separate
 // reduction launch):  out[v] = sum_b partial[b * stride + off + v],  v < nvals <= blockDim.x.
 // Thread (g, v) sums the rows b = g, g+G, ... (coalesced in v), then the G group sums are added in fixed order.
