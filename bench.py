@@ -207,6 +207,7 @@ def main():
     # ---- end to end through the public API with HOST buffers: set_initial(host) + K steps + moments() each
     # step (device->host read of the diagnostics) + get_factors(host) at the end, all inside the timed region
     Xp, Sp, Vp = (torch.from_numpy(np.ascontiguousarray(a.T)).pin_memory() for a in (X, S, V))
+    Xo, So, Vo = (torch.empty_like(t).pin_memory() for t in (Xp, Sp, Vp))      # pinned destination of get_factors
     e2e_steps = max(1, min(args.steps, 10))
     barrier()
     t0 = time.perf_counter()
@@ -214,7 +215,7 @@ def main():
     for _ in range(e2e_steps):
         ctx.step(tau)
         ctx.moments()
-    ctx.get_factors()
+    ctx.get_factors(out=(Xo, So, Vo))
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     fac_bytes = (X.nbytes + S.nbytes + V.nbytes)
@@ -251,7 +252,7 @@ def main():
                              "two-stream f0): another machine and initial value, context only",
             "clocks": summarize_clocks(samples),
             "e2e": {"value": e2e_ms, "unit": "ms/step", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "what": f"set_initial(pinned host)+{e2e_steps}x(dlr_step+dlr_moments)+get_factors(host), per step"},
+                    "what": f"set_initial(pinned host)+{e2e_steps}x(dlr_step+dlr_moments)+get_factors(pinned host), per step"},
             "gpu_launches": launches * args.steps,
             "launches_per_step": launches,
             "roofline": roofline,

@@ -164,7 +164,13 @@ class Dlr:
                "nonfinite": m.nonfinite}
         return (out, f) if npb else out
 
-    def get_factors(self):
+    def get_factors(self, out=None):
+        """(X, S, V) as Fortran-ordered numpy arrays; with out = (X, S, V) host tensors/arrays of r*N, r*r, r*N doubles
+        in the ABI's column-major layout (e.g. pinned torch tensors of shape (r, N)) the copy goes there instead"""
+        if out is not None:
+            X, S, V = out
+            self._check(lib().dlr_get_factors(self.h, _ptr(X), _ptr(S), _ptr(V), 0), "dlr_get_factors")
+            return out
         X = np.empty((self.Nx, self.r), order="F")
         S = np.empty((self.r, self.r), order="F")
         V = np.empty((self.Nv, self.r), order="F")
