@@ -237,6 +237,64 @@ def test_config5_invariants():
     ctx.close()
 
 
+def test_bit_reproducible_and_reinitialisable():
+    """all reductions are fixed-order (per-CTA rows, group sums, single-CTA consumers; no atomics on data), so two
+    contexts fed the same inputs agree BIT FOR BIT; the same holds for one context after dlr_set_initial is called
+    again (the cached C coefficients, the warm-started eigenvectors and the step graph must not leak state)."""
+    cfg = inputs.make_config(1, n=16, r=10)
+    X, S, V = inputs.initial_factors(cfg)
+    a, b = make_ctx(cfg), make_ctx(cfg)
+    outs = []
+    for ctx in (a, b):
+        ctx.set_initial(X, S, V)
+        for _ in range(4):
+            ctx.step(cfg["tau"])
+        outs.append(ctx.get_factors())
+    for u, w in zip(*outs):
+        assert np.array_equal(u, w)
+    a.set_initial(X, S, V)                       # again on a used context
+    for _ in range(4):
+        a.step(cfg["tau"])
+    for u, w in zip(a.get_factors(), outs[0]):
+        assert np.array_equal(u, w)
+    a.close()
+    b.close()
+
+
+def test_step_size_change_recaptures_the_graph():
+    """tau may change from call to call (the step graph is re-captured and the tables rebuilt): steps of size
+    tau, tau/2, tau/2, tau against the oracle doing the same"""
+    cfg = inputs.make_config(1, n=16, r=8)
+    gx, gv = grids(cfg)
+    X, S, V = inputs.initial_factors(cfg)
+    ix, iv = inputs.probe_indices(cfg)
+    ctx = make_ctx(cfg)
+    ctx.set_initial(X, S, V)
+    for tau in (0.1, 0.05, 0.05, 0.1):
+        ctx.step(tau)
+        X, S, V = O.step_alg2(X, S, V, tau, gx, gv)
+        check(ctx, X, S, V, gx, gv, ix, iv, TOL_STEP)
+    ctx.close()
+
+
+def test_strongly_anisotropic_grids():
+    """n_x << n_v and n_x >> n_v (the paper's headline shape is 64^3 x 256^3): different tile shapes,
+    tables and FFT plans on the two grids inside one step; both orders"""
+    for n_x, n_v, order in ((8, 32, 2), (32, 8, 2), (8, 32, 1)):
+        cfg = inputs.make_config(2, n_x=n_x, n_v=n_v, r=8)
+        gx, gv = grids(cfg)
+        X, S, V = inputs.initial_factors(cfg)
+        ix, iv = inputs.probe_indices(cfg)
+        ctx = make_ctx(cfg, order)
+        ctx.set_initial(X, S, V)
+        step = O.step_alg2 if order == 2 else O.step_alg1
+        for _ in range(2):
+            ctx.step(0.1)
+            X, S, V = step(X, S, V, 0.1, gx, gv)
+            check(ctx, X, S, V, gx, gv, ix, iv, TOL_STEP)
+        ctx.close()
+
+
 def test_error_codes():
     from paper_2110_13481_b200 import dlr
     cfg = inputs.make_config(1)
