@@ -77,7 +77,7 @@ def kernel_breakdown(ctx, tau, cfg, nprof=5):
     ctx.set_profiling(0)
     names = [n for n, _ in runs[0]]
     ms = np.median(np.array([[t for _, t in r] for r in runs]), axis=0)
-    B = 8.0 * cfg["n_x"] ** 3 * cfg["r"]
+    B = 8.0 * (0.5 * (cfg["n_x"] ** 3 + cfg["n_v"] ** 3)) * cfg["r"]     # x and v passes alternate: mean factor size
     EN = 8.0 * cfg["n_x"] ** 3
     fam = {}
     total = float(sum(t for t in ms if t > 0))
@@ -129,6 +129,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours")
+    ap.add_argument("--n-x", type=int, default=0, help="override the x grid of --config (the paper's anisotropic shapes)")
+    ap.add_argument("--n-v", type=int, default=0, help="override the v grid of --config")
+    ap.add_argument("--rank", type=int, default=0, help="override the rank of --config")
     ap.add_argument("--cpu-steps", type=int, default=1, help="oracle steps timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -137,7 +140,14 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
     from paper_2110_13481_b200 import inputs
-    cfg = inputs.make_config(args.config)
+    over = {}
+    if args.n_x:
+        over["n_x"] = args.n_x
+    if args.n_v:
+        over["n_v"] = args.n_v
+    if args.rank:
+        over["r"] = args.rank
+    cfg = inputs.make_config(args.config, **over)
     workload = (f"BASELINE.json configs[{args.config - 1}]: {cfg['problem']} {cfg['n_x']}^3x{cfg['n_v']}^3, r={cfg['r']}, "
                 f"tau={cfg['tau']}, Algorithm 2")
     config = {"workload": workload, "n": cfg["n"], "rank": cfg["r"], "tau": cfg["tau"], "parallelism": f"replicas x{args.gpus}",
