@@ -60,7 +60,7 @@ __host__ inline size_t d1_smem_bytes(int n, int RMAX, int T, bool needE, int nma
 }
 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
-__global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 10 ? 2 : 1)) k_d1(const D1Args a) {
+__global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 16 ? 2 : 1)) k_d1(const D1Args a) {
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
     constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : 0;
     const int n = a.g.n, M = n >> 1, lg = a.g.log2n, logM = lg - 1, T = a.T;
