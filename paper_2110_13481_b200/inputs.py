@@ -25,6 +25,10 @@ CONFIGS = {
             alpha=0.5, kappa=0.5, tau=0.05, steps=50),
     5: dict(n=256, r=20, x_lo=0.0, x_hi=4 * math.pi, v_lo=-6.0, v_hi=6.0, problem="landau",
             alpha=0.01, kappa=0.5, tau=0.05, steps=10, rank20_amp=1e-6, band=4),
+    # not a BASELINE.json config: the paper's own two-stream initial value, eq. (21), the workload of
+    # its Table 4 and Section 6.3: v_bar = (5/2, 0, 0), v_tilde = (-5/2, -9/4, -2), norm 1/sqrt((8 pi)^3)
+    6: dict(n=64, r=10, x_lo=0.0, x_hi=10 * math.pi, v_lo=-9.0, v_hi=9.0, problem="twostream_paper",
+            alpha=1e-3, kappa=0.2, v_bar=(2.5, 0.0, 0.0), v_til=(-2.5, -2.25, -2.0), tau=0.01, steps=100),
 }
 
 
@@ -93,6 +97,10 @@ def initial_factors(cfg):
         v0 = cfg["v0"]
         b1 = 0.5 * (np.exp(-0.5 * (v - v0) ** 2) + np.exp(-0.5 * (v + v0) ** 2)) / math.sqrt(TWO_PI)
         M = _outer3(b1, m1, m1)
+    elif cfg["problem"] == "twostream_paper":
+        b = [(np.exp(-0.5 * (v - vb) ** 2) + np.exp(-0.5 * (v - vt) ** 2)) / math.sqrt(4.0 * TWO_PI)
+             for vb, vt in zip(cfg["v_bar"], cfg["v_til"])]
+        M = _outer3(b[0], b[1], b[2])
     else:
         raise ValueError(cfg["problem"])
     rng = np.random.default_rng(cfg["seed"])

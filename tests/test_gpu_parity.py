@@ -360,6 +360,28 @@ def test_paper_linear_landau_headline_shape():
     assert en_err < 1e-5
 
 
+def test_paper_two_stream_initial_value():
+    """the paper's own two-stream initial value, eq. (21) (inputs config 6): beams at different
+    velocities in all three directions, so every momentum component and all three real-space terms are exercised.
+    Closed forms at t = 0 (mass L^3, momentum = mean beam velocity x mass), then two steps against the oracle."""
+    cfg = inputs.make_config(6, n=16, r=10, tau=0.01)
+    gx, gv = grids(cfg)
+    X, S, V = inputs.initial_factors(cfg)
+    ix, iv = inputs.probe_indices(cfg)
+    ctx = make_ctx(cfg)
+    ctx.set_initial(X, S, V)
+    m = ctx.moments()
+    mass = (10 * math.pi) ** 3
+    assert rel(m["mass"], mass) <= 1e-5                      # 16-point quadrature of the Gaussians
+    for d, vmean in enumerate((0.0, -1.125, -1.0)):
+        assert abs(m["momentum"][d] - vmean * mass) <= 1e-4 * mass
+    for _ in range(2):
+        ctx.step(cfg["tau"])
+        X, S, V = O.step_alg2(X, S, V, cfg["tau"], gx, gv)
+        check(ctx, X, S, V, gx, gv, ix, iv, TOL_STEP)
+    ctx.close()
+
+
 def test_error_codes():
     from paper_2110_13481_b200 import dlr
     cfg = inputs.make_config(1)
