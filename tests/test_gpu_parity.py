@@ -382,6 +382,41 @@ def test_paper_two_stream_initial_value():
     ctx.close()
 
 
+def test_paper_two_stream_instability_128():
+    """Section 6.3 of the paper (Fig. 5): two-stream instability (eq. (21)) on 128^3 x 128^3, r = 10,
+    tau = 0.06 up to T = 60 (1000 steps of Algorithm 2).  The paper prints no numbers, only the behaviour: "the electric
+    energy shows an exponential increase before entering into a saturation phase", mass and energy errors grow in the
+    nonlinear phase.  Checked here: growth by more than four orders of magnitude that is exponential (straight in
+    log scale over t in [15, 30]), saturation afterwards, errors bounded, no QR repair, nothing non-finite."""
+    cfg = inputs.make_config(6, n_x=128, n_v=128, r=10)
+    X, S, V = inputs.initial_factors(cfg)
+    ctx = make_ctx(cfg)
+    ctx.set_initial(X, S, V)
+    del X, V
+    tau, nsteps = 0.06, 1000
+    m0 = ctx.moments()
+    e0 = m0["kinetic_energy"] + m0["electric_energy"]
+    t, ee, worst = [], [], 0.0
+    for i in range(1, nsteps + 1):
+        ctx.step(tau)
+        if i % 10 == 0:
+            m = ctx.moments()
+            t.append(i * tau)
+            ee.append(m["electric_energy"])
+            worst = max(worst, rel(m["mass"], m0["mass"]), rel(m["kinetic_energy"] + m["electric_energy"], e0))
+            assert m["qr_fallbacks"] == 0 and m["nonfinite"] == 0
+    ctx.close()
+    t, ee = np.array(t), np.array(ee)
+    assert ee.max() > 1e4 * ee[t < 10].min()
+    lin = (t >= 15) & (t <= 30)
+    slope, icpt = np.polyfit(t[lin], np.log(ee[lin]), 1)
+    assert 0.3 < slope < 0.7
+    assert np.abs(np.log(ee[lin]) - (slope * t[lin] + icpt)).max() < 0.5          # exponential growth
+    sat = ee[t > 36]
+    assert sat.max() < 3.0 * sat.min()                                             # saturation
+    assert worst < 2e-2
+
+
 def test_error_codes():
     from paper_2110_13481_b200 import dlr
     cfg = inputs.make_config(1)
