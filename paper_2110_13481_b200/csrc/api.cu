@@ -740,7 +740,7 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e == cudaSuccess) e = cudaMemsetAsync(c->status, 0, 4 * sizeof(int), c->st);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->grp_cnt, 0, 3 * DLR_CNT_STRIDE * sizeof(unsigned), c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-    if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
+    if (e != cudaSuccess) { dlr_destroy(c); return DLR_ERR_CUDA; }      // releases the streams and events created above
     *out = c;
     return DLR_OK;
 }
