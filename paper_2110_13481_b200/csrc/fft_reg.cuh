@@ -130,7 +130,8 @@ __device__ __forceinline__ void fft_mid_group(double2* s, int LP, FastDiv nl, in
 // all groups of the forward (or inverse) transform; skip_last omits the LAST forward group / the FIRST inverse group
 // (they are done by fft_mid).  Every group ends with a __syncthreads().
 template <bool INV>
-__device__ __forceinline__ void fft_lines_c(double2* s, int LP, int nlines, int logM, bool skip_last) {
+__device__ __forceinline__ void fft_lines_c(double2* s, int LP, int nlines, int logM, bool skip_last,
+                                            bool skip_first = false) {
     int g[3], ng;
     fft_plan(logM, g, ng);
     const FastDiv nl = make_fastdiv((unsigned)nlines);
@@ -141,6 +142,7 @@ __device__ __forceinline__ void fft_lines_c(double2* s, int LP, int nlines, int 
     for (int ii = 0; ii < ng; ii++) {
         const int i = INV ? ng - 1 - ii : ii;
         if (skip_last && i == ng - 1) continue;
+        if (skip_first && i == 0) continue;
         switch (g[i]) {
             case 1: fft_group_c<1, INV>(s, LP, nl, logM, lev[i]); break;
             case 2: fft_group_c<2, INV>(s, LP, nl, logM, lev[i]); break;
@@ -203,5 +205,69 @@ __device__ __forceinline__ void fft_mid2(double2* s, int boff, int LP, int nline
         case 2: fft_mid2_group<2, FA, FB, IA, IB, SA, SB>(s, boff, LP, nl, logM, f); break;
         default: fft_mid2_group<3, FA, FB, IA, IB, SA, SB>(s, boff, LP, nl, logM, f); break;
     }
+    __syncthreads();
+}
+
+// First forward group fed from GLOBAL memory and last inverse group writing to GLOBAL memory (passes whose tile needs no
+// point-wise work across columns before / after the transform: the direction-2 sub-flow, the Parseval-only coefficient
+// passes): the tile makes two round trips through shared memory instead of four.  IDX(e, l) = global double2 index
+// (within one column) of tile element (e, l); column stride N2; line = c * L + l.  Only for transforms of >= 2 groups.
+template <int G, class IDX>
+__device__ __forceinline__ void fft_first_from_global(const double2* __restrict__ in2, size_t N2, IDX idx, double2* s,
+                                                      int LP, FastDiv nl, int logM, int L, int lL) {
+    constexpr int R = 1 << G;
+    const int nlines = (int)nl.d;
+    const int logst = logM - G, st = 1 << logst;
+    const int items = st * nlines;
+    for (int w = threadIdx.x; w < items; w += blockDim.x) {
+        const int j = (int)fdiv((unsigned)w, nl);
+        const int line = w - j * nlines;
+        const int c = line >> lL, l = line & (L - 1);
+        const double2* src = in2 + (size_t)c * N2;
+        double2 a[R];
+#pragma unroll
+        for (int q = 0; q < R; q++) a[q] = src[idx(j + q * st, l)];
+        bfly<G, false>(a);
+#pragma unroll
+        for (int q = 1; q < R; q++) a[q] = cmul(a[q], tw_const(j * brev_small(q, G), logM));
+        double2* p = s + (size_t)j * LP + line;
+#pragma unroll
+        for (int q = 0; q < R; q++) p[(size_t)q * st * LP] = a[q];
+    }
+}
+
+template <int G, class IDX>
+__device__ __forceinline__ void fft_last_to_global(const double2* s, int LP, FastDiv nl, int logM, int L, int lL,
+                                                   double2* __restrict__ out2, size_t N2, IDX idx) {
+    constexpr int R = 1 << G;
+    const int nlines = (int)nl.d;
+    const int logst = logM - G, st = 1 << logst;
+    const int items = st * nlines;
+    for (int w = threadIdx.x; w < items; w += blockDim.x) {
+        const int j = (int)fdiv((unsigned)w, nl);
+        const int line = w - j * nlines;
+        const int c = line >> lL, l = line & (L - 1);
+        const double2* p = s + (size_t)j * LP + line;
+        double2 a[R];
+#pragma unroll
+        for (int q = 0; q < R; q++) a[q] = p[(size_t)q * st * LP];
+#pragma unroll
+        for (int q = 1; q < R; q++) a[q] = cmulc(a[q], tw_const(j * brev_small(q, G), logM));
+        bfly<G, true>(a);
+        double2* dst = out2 + (size_t)c * N2;
+#pragma unroll
+        for (int q = 0; q < R; q++) dst[idx(j + q * st, l)] = a[q];
+    }
+}
+
+// the groups between the first and the last one (only transforms of three groups have one); ends with a barrier
+template <bool INV>
+__device__ __forceinline__ void fft_middle_groups_c(double2* s, int LP, int nlines, int logM) {
+    int g[3], ng;
+    fft_plan(logM, g, ng);
+    if (ng < 3) return;
+    const FastDiv nl = make_fastdiv((unsigned)nlines);
+    if (g[1] == 2) fft_group_c<2, INV>(s, LP, nl, logM, g[0]);
+    else fft_group_c<3, INV>(s, LP, nl, logM, g[0]);
     __syncthreads();
 }

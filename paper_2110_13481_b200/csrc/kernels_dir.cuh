@@ -205,8 +205,19 @@ k_dir(const DirArgs a) {
     const size_t N2 = (size_t)(a.g.N >> 1);
     const double invn = 1.0 / (double)n;
 
+    // Passes without point-wise work across the columns before the transform (direction-2 sub-flow, Parseval-only
+    // coefficient passes) feed the first FFT group straight from global memory (and the sub-flow writes its last inverse
+    // group straight back): two round trips through shared memory instead of four.  Needs a transform of >= 2 groups.
+    constexpr bool GLOBAL_FFT = (DOP == DOP_EXACT && DIR == 2) || (DOP == DOP_COEFF && DW == DW_NONE && DIR != 1);
+    const bool gfft = GLOBAL_FFT && lg >= 4;
+    const auto gidx = [&](int e, int l) { return dir_index<DIR>(gm, e, l); };
+    const FastDiv fnl = make_fastdiv((unsigned)nl);
+    if (gfft) {
+        if (lg == 4) fft_first_from_global<2>((const double2*)a.in, N2, gidx, z, LPZ, fnl, lg, L, lL);
+        else fft_first_from_global<3>((const double2*)a.in, N2, gidx, z, LPZ, fnl, lg, L, lL);
+    }
     // ------------------------------------------------------------------ load
-    {
+    if (!gfft) {
         const double2* in2 = (const double2*)a.in;
         if (DIR == 1) {
             const int lM = lg - 1, items = nl << lM;
@@ -270,7 +281,7 @@ k_dir(const DirArgs a) {
                 gw.acc, gw.cs);
             __syncthreads();
         }
-        fft_lines_c<false>(z, LPZ, nl, lg, false);
+        fft_lines_c<false>(z, LPZ, nl, lg, false, gfft);       // (the first group is already done when fed from global)
         double pacc[NTP][2];
 #pragma unroll
         for (int t = 0; t < NTP; t++) pacc[t][0] = pacc[t][1] = 0.0;
@@ -326,7 +337,7 @@ k_dir(const DirArgs a) {
             }
             __syncthreads();
         }
-        fft_lines_c<false>(z, LPZ, nl, lg, true);
+        fft_lines_c<false>(z, LPZ, nl, lg, true, gfft);
         {
             const double2* ph = a.ph;
             fft_mid(z, LPZ, nl, lg, [&](double2& v, int e, int line) {
@@ -335,7 +346,12 @@ k_dir(const DirArgs a) {
                 v = cmul(v, f);
             });
         }
-        fft_lines_c<true>(z, LPZ, nl, lg, true);
+        fft_lines_c<true>(z, LPZ, nl, lg, true, gfft);
+        if (gfft) {                                           // last inverse group straight to global memory: done
+            if (lg == 4) fft_last_to_global<2>(z, LPZ, fnl, lg, L, lL, (double2*)a.out, N2, gidx);
+            else fft_last_to_global<3>(z, LPZ, fnl, lg, L, lL, (double2*)a.out, N2, gidx);
+            return;
+        }
         if (MIX && a.mout != nullptr) {
             for (int w = tid; w < pitems; w += nth) {
                 const int l = w & (L - 1), e = w >> lL;
