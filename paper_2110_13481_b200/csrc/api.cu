@@ -74,6 +74,7 @@ struct dlr_ctx {
     double2* Eh;
     double *KL, *Q1, *W, *E;
     double *partial, *partialP[3], *partialC, *partial2a;
+    double *margp1, *margp2, *margV;         // marginals of V (k_marginals partial planes; M1, M2, M3 as 3 x [r][n_v])
     double *gram2, *pgram2[3], *colsum2;     // group sums of the per-CTA partial rows (group_prereduce)
     unsigned* grp_cnt;                       // 3 x DLR_CNT_STRIDE group counters, zero between kernels
     // small buffers
@@ -231,6 +232,12 @@ size_t carve(dlr_ctx* c, char* base) {
     for (int d = 0; d < 3; d++) c->pgram2[d] = cv.take<double>(groups * (size_t)(R * (R - 1) / 2));
     c->colsum2 = cv.take<double>(groups * (size_t)R);
     c->grp_cnt = cv.take<unsigned>(3 * DLR_CNT_STRIDE);
+    {
+        const size_t nv = (size_t)c->gv.g.n;
+        c->margp1 = cv.take<double>((size_t)R * nv * nv);
+        c->margp2 = cv.take<double>((size_t)R * nv * nv);
+        c->margV = cv.take<double>(3 * (size_t)R * nv);
+    }
     c->partial2a = cv.take<double>((size_t)DLR_G1 * nvmax);
     const int RR = R * R;
     c->S = cv.take<double>(RR); c->Sp = cv.take<double>(RR);
@@ -439,6 +446,36 @@ void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M
     c->count_launches -= 1;
 }
 
+// 1D marginals of V for the flow-free predictor L step (k_lpred_sums): one light read-only pass and a reduction.
+// Called wherever the C coefficients of V are computed (V changes only at the L-step QR).
+void marginals_V(dlr_ctx* c) {
+    const HostGrid& hg = c->gv;
+    const int n = hg.g.n, R = c->R;
+    k_marginals<<<dim3(n, R), 256, 0, c->st>>>(c->V, hg.g, c->margp1, c->margp2);
+    CK(cudaGetLastError());
+    k_marg_reduce<<<dim3(R, 3), 256, 0, c->st>>>(c->margp1, c->margp2, n, c->margV, c->margV + (size_t)R * n,
+                                         c->margV + 2 * (size_t)R * n);
+    CK(cudaGetLastError());
+    c->bytes_acc += fac_bytes(c, hg);
+}
+
+// Column sums of the predictor's L1 (all that line 2 of Algorithm 2 needs of it) from the marginals of V and the tables
+// of the L-flow that post() has just built.
+void lpred_sums(dlr_ctx* c, double t3) {
+    const HostGrid& hg = c->gv;
+    const size_t n = (size_t)hg.g.n, R = (size_t)c->R;
+    const size_t sm = n * 16 + n * R * 16 + n * R * 8 + R * R * 8 + 8 * R * 8 + (7 * R * R + 1) * 8 + n * 16 + 64;
+    static size_t configured = 0;
+    if (sm > configured) {
+        CK(cudaFuncSetAttribute(k_lpred_sums, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        c->count_launches--;
+        configured = sm;
+    }
+    k_lpred_sums<<<1, DLR_SMALL_THREADS, sm, c->st>>>(c->margV, c->margV + R * n, c->margV + 2 * R * n, (int)R, hg.g,
+                                                      c->ft.p, t3, c->zsum);
+    CK(cudaGetLastError());
+}
+
 // The r x r work between two streaming phases, one launch (see k_post).
 struct PostM2 { const HostGrid* hg; double* M2; };
 struct PostS { double* S; double t; };
@@ -587,6 +624,7 @@ void issue_step(dlr_ctx* c, double tau) {
     // ---- Algorithm 1, line 1: C coefficients from V0 (kept from the previous step's line 10 when valid)
     if (!c->vh_valid) {
         coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
+        marginals_V(c);
         post(c, &m2C, nullptr, nullptr);
     }
     phase_mark(c, "C coefficients (V0)");
@@ -623,7 +661,7 @@ void issue_step(dlr_ctx* c, double tau) {
         c->bytes_step = c->bytes_acc;
         return;
     }
-    flow(c, gv, c->V, true, 1, true);            // only rho(L1) = L1^T omega_v is needed (eq. (13))
+    lpred_sums(c, tp);                           // only rho(L1) = L1^T omega_v is needed (eq. (13)): no flow, see k_lpred_sums
     phase_mark(c, "L step (predictor)");
     // ---- Algorithm 2, line 2: E^{1/2} from X1 and L1, eq. (13)
     field_fork(c, Xp, nullptr, c->zsum, 1, -gv.g.h3);
@@ -654,6 +692,7 @@ void issue_step(dlr_ctx* c, double tau) {
     // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step;
     //      tables of the second K step (K3 = X2 S6)
     coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
+    marginals_V(c);
     phase_mark(c, "C coefficients");
     {
         const PostS sf{c->S, 0.5 * tau};

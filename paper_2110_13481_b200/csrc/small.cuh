@@ -629,3 +629,187 @@ __global__ void k_probes(const double* X, const double* S, const double* V, long
     }
     f[p] = s;
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// Predictor L step of Algorithm 2 without the flow.  Line 2 of Algorithm 2 needs of L1 only its column sums
+// (rho = -X (L^T omega_v), eq. (13)).  Every operation of the Lie L-flow is linear and separable:
+// the exact sub-flow along direction d preserves the marginal sums over the other directions and acts on the marginal
+// along d as the same 1D shift; the exponential-Euler stage changes the total only by t * sum_points N(m), and
+// N(m) = sum_i v_i o (m Q_i) needs the first moments sum_points v_i m only.  So the column sums of L1 follow from the three
+// 1D marginals of V (3 n r numbers), n-point DFTs and r x r products - mathematically the same numbers as the full flow.
+//
+// k_marginals: grid (n, R): CTA (i3, c) sums the plane (i1, i2) of column c:  p1[(c n + i3) n + i1] = sum_i2 A,
+//              p2[(c n + i3) n + i2] = sum_i1 A.   k_marg_reduce: M1[c][i1], M2[c][i2] = sums over i3; M3[c][i3] = sum_i2 p2.
+__global__ void __launch_bounds__(256) k_marginals(const double* A, GridDev g, double* p1, double* p2) {
+    __shared__ double cs[8][256];
+    const int n = g.n, lg = g.log2n, i3 = blockIdx.x, c = blockIdx.y;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const double* plane = A + (size_t)c * g.N + ((size_t)i3 << (2 * lg));
+    double col[8] = {0, 0, 0, 0, 0, 0, 0, 0};                    // column sums of this warp's rows, i1 = lane + 32 k
+    double* row2 = p2 + ((size_t)c * n + i3) * n;
+    for (int i2 = w; i2 < n; i2 += nw) {
+        const double* row = plane + ((size_t)i2 << lg);
+        double rs = 0.0;
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            const int i1 = lane + 32 * k;
+            if (i1 < n) { const double v = row[i1]; col[k] += v; rs += v; }
+        }
+        rs = warp_sum(rs);
+        if (lane == 0) row2[i2] = rs;
+    }
+#pragma unroll
+    for (int k = 0; k < 8; k++) cs[w][lane + 32 * k] = col[k];
+    __syncthreads();
+    for (int i1 = threadIdx.x; i1 < n; i1 += blockDim.x) {
+        double s = 0.0;
+        for (int ww = 0; ww < nw; ww++) s += cs[ww][i1];
+        p1[((size_t)c * n + i3) * n + i1] = s;
+    }
+}
+
+// grid (R, 3): CTA (c, which).  which 0, 1: M[c][i] = sum_k p[(c n + k) n + i] (coalesced in i, four k-groups per i);
+// which 2: M3[c][i3] = sum_i2 p2[(c n + i3) n + i2] (one warp per row, lanes along i2).
+__global__ void __launch_bounds__(256) k_marg_reduce(const double* p1, const double* p2, int n, double* M1, double* M2,
+                                                     double* M3) {
+    __shared__ double red[256];
+    const int c = blockIdx.x, which = blockIdx.y, tid = threadIdx.x;
+    if (which < 2) {
+        const double* p = (which == 0 ? p1 : p2) + (size_t)c * n * n;
+        double* M = (which == 0 ? M1 : M2) + (size_t)c * n;
+        const int ng = max(1, (int)blockDim.x / n);              // k-groups
+        for (int i0 = 0; i0 < n; i0 += blockDim.x) {
+            const int i = i0 + (tid % n), kg = tid / n;
+            double s = 0.0;
+            if (i < n && kg < ng)
+                for (int k = kg; k < n; k += ng) s += p[(size_t)k * n + i];
+            red[tid] = s;
+            __syncthreads();
+            if (tid < n && i0 + tid < n) {
+                double t = 0.0;
+                for (int gq = 0; gq < ng; gq++) t += red[gq * n + tid];
+                M[i0 + tid] = t;
+            }
+            __syncthreads();
+        }
+    } else {
+        const int lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
+        for (int i = w; i < n; i += nw) {
+            const double* row = p2 + ((size_t)c * n + i) * n;
+            double s = 0.0;
+            for (int k = lane; k < n; k += 32) s += row[k];
+            s = warp_sum(s);
+            if (lane == 0) M3[(size_t)c * n + i] = s;
+        }
+    }
+}
+
+// column sums of the predictor's L1 from the marginals (see above); single CTA.  mats/Q/ph1/ph2: the tables of the
+// L-flow built by k_post (FlowTabPtrs), t3 = length of the third sub-flow.  zsum[c] = sum_points L1_c (no h^3 weight).
+__global__ void __launch_bounds__(DLR_SMALL_THREADS)
+k_lpred_sums(const double* M1, const double* M2, const double* M3, int R, GridDev g, FlowTabPtrs tb, double t3,
+             double* zsum) {
+    extern __shared__ double2 lsm[];
+    const int n = g.n, lg = g.log2n, RR = R * R, tid = threadIdx.x, nth = blockDim.x;
+    double2* W = lsm;                                   // [n]  sum_i v(i) e^{+2 pi i ik/n}
+    double2* part = W + n;                              // [n][R] terms of the moment sums
+    double* F = (double*)(part + (size_t)n * R);        // [n][R] mixed marginal
+    double* B = F + (size_t)n * R;                      // [R][R] A0 or A0 A1
+    double* vec = B + RR;                               // 8 x [R] small vectors
+    double *s0 = vec, *mom3 = vec + R, *nu1 = vec + 2 * R, *nu2 = vec + 3 * R, *ta = vec + 4 * R, *tb2 = vec + 5 * R,
+           *acc = vec + 6 * R, *tmpv = vec + 7 * R;
+    double* msm = vec + 8 * R;                          // [7][R][R]: A0, A1, A2, A3, Q1..3 (one parallel load)
+    double2* twf = (double2*)(msm + 7 * RR);             // [n] exp(-2 pi i m / n), full circle (8 R (R + 1) doubles after B: 16-byte aligned)
+    for (int i = tid; i < 4 * RR; i += nth) msm[i] = tb.mats[i];
+    for (int i = tid; i < 3 * RR; i += nth) msm[4 * RR + i] = tb.Q[i];
+    for (int m = tid; m < n; m += nth) {
+        const double2 w = m < (n >> 1) ? g.tw[m] : g.tw[m - (n >> 1)];
+        twf[m] = m < (n >> 1) ? w : make_double2(-w.x, -w.y);
+    }
+    __syncthreads();
+    const double* A0 = msm;
+    const double* A1 = msm + RR;
+    const double* A2 = msm + 2 * RR;
+    const double* A3 = msm + 3 * RR;
+    const double* Qs = msm + 4 * RR;
+    auto twd = [&](int m) { return twf[m]; };            // exp(-2 pi i m / n), 0 <= m < n
+    for (int k = tid; k < n; k += nth) {
+        double2 s = make_double2(0.0, 0.0);
+        for (int i = 0; i < n; i++) {
+            const double2 w = twd((i * k) & (n - 1));
+            const double v = g.lo + g.h * i;
+            s.x = fma(v, w.x, s.x);
+            s.y = fma(v, -w.y, s.y);                     // conjugate: e^{+...}
+        }
+        W[k] = s;
+    }
+    if (tid < R) {
+        double a = 0.0, b = 0.0;
+        for (int i = 0; i < n; i++) {
+            a += M1[(size_t)tid * n + i];
+            b = fma(g.lo + g.h * i, M3[(size_t)tid * n + i], b);
+        }
+        s0[tid] = a;
+        mom3[tid] = b;
+    }
+    __syncthreads();
+    for (int d = 0; d < 2; d++) {
+        // B = A0 (direction 1) or A0 A1 (direction 2);  F = P_d B;  nu_d[c] = (1/n) Re sum_k ph_d[k][c] F^_k[c] W_k
+        for (int idx = tid; idx < RR; idx += nth) {
+            const int a = idx / R, b = idx - a * R;
+            double s = A0[idx];
+            if (d == 1) { s = 0.0; for (int k = 0; k < R; k++) s = fma(A0[a * R + k], A1[k * R + b], s); }
+            B[idx] = s;
+        }
+        __syncthreads();
+        const double* P = d == 0 ? M1 : M2;
+        for (int idx = tid; idx < n * R; idx += nth) {
+            const int i = idx / R, c = idx - i * R;
+            double s = 0.0;
+            for (int k = 0; k < R; k++) s = fma(P[(size_t)k * n + i], B[k * R + c], s);
+            F[idx] = s;
+        }
+        __syncthreads();
+        const double2* ph = d == 0 ? tb.ph1 : tb.ph2;
+        for (int idx = tid; idx < n * R; idx += nth) {
+            const int k = idx / R, c = idx - k * R;
+            double2 fh = make_double2(0.0, 0.0);
+            for (int i = 0; i < n; i++) {
+                const double2 w = twd((i * k) & (n - 1));
+                const double f = F[i * R + c];
+                fh.x = fma(f, w.x, fh.x);
+                fh.y = fma(f, w.y, fh.y);
+            }
+            const int ep = (int)(__brev((unsigned)k) >> (32 - lg));           // stored position of wavenumber index k
+            part[idx] = cmul(cmul(ph[(size_t)ep * R + c], fh), W[k]);
+        }
+        __syncthreads();
+        if (tid < R) {
+            double s = 0.0;
+            for (int k = 0; k < n; k++) s += part[k * R + tid].x;
+            (d == 0 ? nu1 : nu2)[tid] = s / (double)n;
+        }
+        __syncthreads();
+    }
+    // r x r chain (row vector times matrix, [cin][cout]), by the first R threads
+    auto vm = [&](const double* v, const double* Mx, double* out) {
+        if (tid < R) {
+            double s = 0.0;
+            for (int k = 0; k < R; k++) s = fma(v[k], Mx[k * R + tid], s);
+            out[tid] = s;
+        }
+        __syncthreads();
+    };
+    vm(s0, A0, ta); vm(ta, A1, tb2); vm(tb2, A2, acc);          // acc = sum_points m
+    vm(mom3, A0, ta); vm(ta, A1, tb2); vm(tb2, A2, mom3);       // mu_3
+    vm(nu2, A2, ta);                                            // mu_2 -> ta
+    vm(nu1, A1, tb2); vm(tb2, A2, nu1);                         // mu_1
+    if (tid < R) {
+        double gsum = 0.0;
+        for (int k = 0; k < R; k++)
+            gsum += nu1[k] * Qs[k * R + tid] + ta[k] * Qs[RR + k * R + tid] + mom3[k] * Qs[2 * RR + k * R + tid];
+        tmpv[tid] = acc[tid] + t3 * gsum;
+    }
+    __syncthreads();
+    vm(tmpv, A3, zsum);
+}
