@@ -63,6 +63,7 @@ struct dlr_ctx {
     cudaStream_t st, cap_st;
     cudaStream_t side;            // side branch: the coefficient/eigen kernel overlaps the dim-2/3 passes of its transform
     cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_mfork;             // marginals of V on the side branch (joined by the coefficient set's join)
     cudaEvent_t ev_ffork, ev_fjoin;   // field solve on the side stream, joined before the first pass that reads E
     bool field_pending;
     bool tc_warm, td_warm;            // TC / TD hold a previous eigen-decomposition (warm start of the Jacobi solves)
@@ -447,13 +448,18 @@ void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M
 }
 
 // 1D marginals of V for the flow-free predictor L step (k_lpred_sums): one light read-only pass and a reduction.
-// Called wherever the C coefficients of V are computed (V changes only at the L-step QR).
+// Called right BEFORE the C coefficients of V are computed (V changes only at the L-step QR): the two kernels go to the
+// side stream, run beside the first coefficient pass, and are covered by the join at the end of coeffs() (the Jacobi
+// kernel follows them on the same stream).
 void marginals_V(dlr_ctx* c) {
     const HostGrid& hg = c->gv;
     const int n = hg.g.n, R = c->R;
-    k_marginals<<<dim3(n, R), 256, 0, c->st>>>(c->V, hg.g, c->margp1, c->margp2);
+    CK(cudaEventRecord(c->ev_mfork, c->st));
+    CK(cudaStreamWaitEvent(c->side, c->ev_mfork, 0));
+    c->count_launches -= 2;
+    k_marginals<<<dim3(n, R), 256, 0, c->side>>>(c->V, hg.g, c->margp1, c->margp2);
     CK(cudaGetLastError());
-    k_marg_reduce<<<dim3(R, 3), 256, 0, c->st>>>(c->margp1, c->margp2, n, c->margV, c->margV + (size_t)R * n,
+    k_marg_reduce<<<dim3(R, 3), 256, 0, c->side>>>(c->margp1, c->margp2, n, c->margV, c->margV + (size_t)R * n,
                                          c->margV + 2 * (size_t)R * n);
     CK(cudaGetLastError());
     c->bytes_acc += fac_bytes(c, hg);
@@ -623,8 +629,8 @@ void issue_step(dlr_ctx* c, double tau) {
     c->bytes_acc = 0.0;
     // ---- Algorithm 1, line 1: C coefficients from V0 (kept from the previous step's line 10 when valid)
     if (!c->vh_valid) {
-        coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
         marginals_V(c);
+        coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
         post(c, &m2C, nullptr, nullptr);
     }
     phase_mark(c, "C coefficients (V0)");
@@ -691,8 +697,8 @@ void issue_step(dlr_ctx* c, double tau) {
     phase_mark(c, "QR L");
     // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step;
     //      tables of the second K step (K3 = X2 S6)
-    coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
     marginals_V(c);
+    coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
     phase_mark(c, "C coefficients");
     {
         const PostS sf{c->S, 0.5 * tau};
@@ -771,6 +777,7 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_mfork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_ffork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fjoin, cudaEventDisableTiming);
     if (e != cudaSuccess) { dlr_destroy(c); return DLR_ERR_CUDA; }
@@ -791,6 +798,7 @@ void dlr_destroy(dlr_ctx* c) {
     if (c->side) cudaStreamDestroy(c->side);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->ev_mfork) cudaEventDestroy(c->ev_mfork);
     if (c->ev_ffork) cudaEventDestroy(c->ev_ffork);
     if (c->ev_fjoin) cudaEventDestroy(c->ev_fjoin);
     for (auto& p : c->phases) cudaEventDestroy(p.ev);
