@@ -249,7 +249,10 @@ def main():
             "launches_per_step": top["launches_per_step"], "share_of_step": top["share_of_step"],
             "note": "dominant kernel family of the step by device time; duration = CUDA events after every launch on "
                     "the context's stream (dlr_set_profiling(ctx, 2), 5 steps, median) right after the timed region; "
-                    "traffic = DRAM bytes per launch from the ncu --set full capture in profiles/ (cold cache)",
+                    "traffic = DRAM bytes per launch from the ncu --set full capture in profiles/ (cold cache). "
+                    "bound = hbm is the roofline the passes are designed against (and what the metric asks for); as "
+                    "measured they are limited by the shared-memory pipe, not by HBM (DRAM traffic = algorithmic bytes, "
+                    "profiles/r01_c_profile_cfg3.md)",
             "step": {"algorithmic_bytes_per_step": bytes_step, "achieved": achieved, "frac": achieved / peak,
                      "what": "all factor-sized passes of one step (DESIGN.md section 6) / CUDA-event time of the step"},
             "kernels": kernels,
