@@ -15,7 +15,8 @@
  *
  * Conventions: C linkage, no exceptions cross the boundary, return 0 = DLR_OK, negative = error.
  * Pointers are HOST pointers unless the argument is documented as device / "on_device".
- * One context per stream/thread; no global state.
+ * One context per stream/thread; no global state: a context lives on the device that owns its workspace (every
+ * call switches to that device and restores the caller's), several contexts of any shape may coexist in a process.
  */
 #ifndef DLR_B200_H
 #define DLR_B200_H
@@ -37,6 +38,12 @@ enum {
     DLR_ERR_NO_STATE = -6          /* dlr_step / dlr_moments before dlr_set_initial */
 };
 
+/* dlr_config.flags: the predictor of Algorithm 2 (line 1) needs of its L step only rho(L^1) = L^1^T omega_v
+ * (eq. (13)), which the default path obtains from the 1D marginals of V without running the flow
+ * (DESIGN.md row a7'). With this flag the Lie L-flow of Algorithm 1 line 9 is run literally and its
+ * column sums are used: same numbers up to rounding, one more pass family per step. For A/B tests. */
+#define DLR_FLAG_PREDICTOR_L_FLOW 1u
+
 /* Grid descriptors of Fig. 2: number of points, left extreme, right extreme of the
  * periodic box per direction (grid spacing h = (hi-lo)/n, points lo + i*h, i = 0..n-1).
  * Supported: n_x[0]=n_x[1]=n_x[2] and n_v[0]=n_v[1]=n_v[2], each a power of two in 8..256 (n_x may differ
@@ -47,7 +54,7 @@ typedef struct dlr_config {
     int32_t rank;
     int32_t order;      /* 2 = Algorithm 2; 1 = Algorithm 1 */
     double e_scale;     /* multiplies the electric field; 1.0 = the paper's equations, 0.0 = test hook "E = 0" */
-    uint32_t flags;     /* reserved, must be 0 */
+    uint32_t flags;     /* 0, or DLR_FLAG_PREDICTOR_L_FLOW */
 } dlr_config;
 
 /* Diagnostics the paper plots (Figs. 4-7). */
@@ -57,8 +64,13 @@ typedef struct dlr_moments_t {
     double kinetic_energy;     /* 1/2 int int |v|^2 f dx dv                                                */
     double electric_energy;    /* 1/2 int |E|^2 dx, E from eq. (12) + Poisson on the state  */
     double s_fro;              /* ||S||_F                                                                   */
-    int32_t qr_fallbacks;      /* number of Cholesky pivots that had to be repaired since dlr_set_initial  */
+    int32_t qr_fallbacks;      /* number of Cholesky pivots that had to be repaired since dlr_set_initial: the
+                                  factor was rank deficient to working precision ("QR or SVD"); 0 in
+                                  every run whose results are compared with the oracle (reading R12)     */
     int32_t nonfinite;         /* 1 if a non-finite value was seen in S                                    */
+    int32_t qr_third_stage;    /* QR decompositions since dlr_set_initial that needed a third CholeskyQR stage
+                                  (kappa(K) >~ 1e7: the first steps of a rank-1 initial value); informational    */
+    int32_t eig_unconverged;   /* symmetric eigen-solves that hit the Jacobi sweep cap; must be 0 */
 } dlr_moments_t;
 
 typedef struct dlr_ctx dlr_ctx;
@@ -95,7 +107,7 @@ int dlr_moments(dlr_ctx* ctx, dlr_moments_t* out, int n_probe, const int64_t* pr
 int dlr_get_factors(dlr_ctx* ctx, double* X, double* S, double* V, int on_device);
 
 /* The electric field used last inside dlr_step (E^{1/2} of Algorithm 2 line 2; E^0 for order 1):
- * 3*N_x doubles, component-major. For tests. */
+ * 3*N_x doubles, component-major. For tests. dlr_moments does not disturb it (its own field buffer). */
 int dlr_get_field(dlr_ctx* ctx, double* E, int on_device);
 
 /* Per-phase device times (ms) of the LAST dlr_step executed with profiling on (dlr_set_profiling(ctx,1)
@@ -120,9 +132,33 @@ double dlr_bytes_per_step(dlr_ctx* ctx);
 int dlr_test_fft_roundtrip(dlr_ctx* ctx, int which, int ncols, const double* d_in, double* d_out,
                            double* d_spec /* 2*ncols*(n/2+1)*n*n doubles */);
 
+/* Kernel-level entry point for tests: ONE directional pass of a K/L flow (section 4) on a factor-
+ * shaped array, so that a parity failure of dlr_step can be located.  d_in, d_out (and d_E: 3*N_x, only which = 0,
+ * kind >= 2): DEVICE arrays of N*r doubles on grid `which` (0 = x, 1 = v); every other pointer is a HOST array.
+ *   kind 0: sub-flow along direction 1, eqs. (14)/(17):  A <- [A min] -> F_1 -> * tabs[k1][j] -> F_1^-1 -> [* mout]
+ *   kind 1: sub-flow along direction 2, eqs. (15)/(18):  F_2 -> * tabs[k2][j] -> F_2^-1     (min, mout ignored)
+ *   kind 2 / 3: third sub-flow, eq. (19), exponential Euler / ETD2RK (reading R8) in a given eigenbasis:
+ *           m = A min; N(m) = sum_i w_i o (m Q_i) with w = E (which = 0) or the velocity coordinate (which = 1);
+ *           tabs = e^z, t phi1, t (phi1 - phi2), t phi2; result times mout.
+ * min, mout: r x r row-major [column in][column out] or NULL (identity); Q: 3 r x r; tabs: complex
+ * [1 or 4][n][r] in NATURAL DFT order of the wavenumber index, conjugate symmetric in k (real lines are transformed
+ * in pairs).  Overwrites the context's flow tables (harmless: every flow of dlr_step rebuilds them). Synchronises. */
+int dlr_test_dir_pass(dlr_ctx* ctx, int which, int kind, const double* d_in, double* d_out, const double* min_,
+                      const double* mout, const double* tabs, const double* Q, const double* d_E);
+
+/* Test entry for the adaptive CholeskyQR: given the upper pairs (row-major, r(r+1)/2 HOST
+ * doubles) of the Gram matrix of a once-orthogonalised factor, reports whether the device-side criterion asks for a
+ * third stage. Does not touch the state or the status counters. */
+int dlr_test_chol_decide(dlr_ctx* ctx, const double* gram_upper, int* third_stage_needed);
+
 void dlr_destroy(dlr_ctx* ctx);
 const char* dlr_strerror(int code);
 const char* dlr_last_cuda_error(dlr_ctx* ctx);
+
+/* After a call returned DLR_ERR_CUDA the context refuses further work until the error is cleared. Clears the
+ * latched error and drops the state (it may be half-updated): dlr_set_initial must follow. A sticky CUDA error
+ * (illegal address, ...) cannot be cleared: the next call fails again. */
+int dlr_clear_error(dlr_ctx* ctx);
 
 #ifdef __cplusplus
 }

@@ -60,6 +60,7 @@ struct Phase {
 struct dlr_ctx {
     dlr_config cfg;
     int R;
+    int dev;                      // device of the workspace: every entry point runs under it (DevGuard)
     cudaStream_t st, cap_st;
     cudaStream_t side;            // side branch: the coefficient/eigen kernel overlaps the dim-2/3 passes of its transform
     cudaEvent_t ev_fork, ev_join;
@@ -74,6 +75,7 @@ struct dlr_ctx {
     double *X, *X1, *V, *S, *Sp;     // X1: the predictor basis of Algorithm 2 (X itself stays X0 until the first K step)
     double2* Eh;
     double *KL, *Q1, *W, *E;
+    double* Em;                   // field of the diagnostics (dlr_moments): c->E stays the field used last by dlr_step
     double *partial, *partialP[3], *partialC, *partial2a;
     double *margp1, *margp2, *margV;         // marginals of V (k_marginals partial planes; M1, M2, M3 as 3 x [r][n_v])
     double *gram2, *pgram2[3], *colsum2;     // group sums of the per-CTA partial rows (group_prereduce)
@@ -103,6 +105,16 @@ namespace {
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// every entry point that touches the device runs with the context's device current and restores the caller's
+struct DevGuard {
+    int prev;
+    bool switched;
+    explicit DevGuard(int dev) : prev(-1), switched(false) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 int ilog2(int n) { int l = 0; while ((1 << l) < n) l++; return l; }
 int brev_host(int k, int bits) { int r = 0; for (int i = 0; i < bits; i++) if (k & (1 << i)) r |= 1 << (bits - 1 - i); return r; }
@@ -131,9 +143,14 @@ int choose_T3(int n, int RMAX, int nmat) {
     return best;
 }
 
-// Tuning overrides for experiments: DLR_TUNE="t1=8,t3=4,nb2=1,smem2=48,thr1=256,thr2=256,thr3=128" (all optional).
+// Tuning overrides for experiments, compiled in only with -DDLR_ENABLE_TUNE (never in the product build):
+// DLR_TUNE="t1=8,t3=4,nb2=1,smem2=48,thr1=256,thr2=256,thr3=128" (all optional).
 // Values are validated by the callers (powers of two, shared-memory limits); unknown keys are ignored.
 int tune(const char* key, int dflt) {
+#ifndef DLR_ENABLE_TUNE
+    (void)key;
+    return dflt;                              // product builds: fixed tile rules, no environment dependence
+#endif
     const char* e = getenv("DLR_TUNE");
     if (!e) return dflt;
     const std::string s(e), k = std::string(key) + "=";
@@ -190,7 +207,7 @@ int check_cfg(const dlr_config* c) {
     if (!is_pow2(nx) || !is_pow2(nv) || nx < 8 || nv < 8 || nx > 256 || nv > 256) return DLR_ERR_UNSUPPORTED;
     if (!dlr_rank_ops(c->rank)) return DLR_ERR_UNSUPPORTED;
     if (c->order != 1 && c->order != 2) return DLR_ERR_INVALID;
-    if (c->flags != 0) return DLR_ERR_INVALID;
+    if ((c->flags & ~(uint32_t)DLR_FLAG_PREDICTOR_L_FLOW) != 0) return DLR_ERR_INVALID;
     for (int d = 0; d < 3; d++) {
         if (!(c->x_hi[d] > c->x_lo[d]) || !(c->v_hi[d] > c->v_lo[d])) return DLR_ERR_INVALID;
         if (c->x_lo[d] != c->x_lo[0] || c->x_hi[d] != c->x_hi[0] || c->v_lo[d] != c->v_lo[0] || c->v_hi[d] != c->v_hi[0])
@@ -214,6 +231,7 @@ size_t carve(dlr_ctx* c, char* base) {
     c->Q1 = cv.take<double>((size_t)Nmax * R);
     c->W = cv.take<double>((size_t)Nmax * R);
     c->E = cv.take<double>((size_t)3 * Nx);
+    c->Em = cv.take<double>((size_t)3 * Nx);
     c->Eh = cv.take<double2>((size_t)3 * NCx);
     // per-CTA partial sums: the largest producer is a dimension-1 pass with the weighted Gram
     const int nvmax = 3 * R * (R + 1) / 2 + R;
@@ -433,7 +451,7 @@ void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M
     CK(cudaEventRecord(c->ev_fork, c->st));
     CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
     k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->gram2, dlr_groups(dir_blocks(hg, hg.Lc)), R, kind == 1, hg.g.h3, M1, colsum, T, lam,
-                                                     (kind == 1 ? c->tc_warm : c->td_warm) ? 1 : 0);
+                                                     (kind == 1 ? c->tc_warm : c->td_warm) ? 1 : 0, c->status);
     CK(cudaGetLastError());
     (kind == 1 ? c->tc_warm : c->td_warm) = true;
     CK(cudaEventRecord(c->ev_join, c->side));
@@ -471,12 +489,6 @@ void lpred_sums(dlr_ctx* c, double t3) {
     const HostGrid& hg = c->gv;
     const size_t n = (size_t)hg.g.n, R = (size_t)c->R;
     const size_t sm = n * 16 + n * R * 16 + n * R * 8 + R * R * 8 + 8 * R * 8 + (7 * R * R + 1) * 8 + n * 16 + 64;
-    static size_t configured = 0;
-    if (sm > configured) {
-        CK(cudaFuncSetAttribute(k_lpred_sums, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-        c->count_launches--;
-        configured = sm;
-    }
     k_lpred_sums<<<1, DLR_SMALL_THREADS, sm, c->st>>>(c->margV, c->margV + R * n, c->margV + 2 * R * n, (int)R, hg.g,
                                                       c->ft.p, t3, c->zsum);
     CK(cudaGetLastError());
@@ -501,12 +513,6 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
         a.sgn = tb->sgn; a.tsub = tb->tsub; a.t3 = tb->t3; a.M2c = tb->M2c; a.nlsign = tb->nlsign; a.o = c->ft.p;
     }
     const size_t sm = sf ? (size_t)12 * c->R * c->R * sizeof(double) : 0;     // staged C1, C2, D1, D2
-    static size_t configured = 0;
-    if (sm > configured) {
-        CK(cudaFuncSetAttribute(k_post, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-        c->count_launches--;
-        configured = sm;
-    }
     k_post<<<1, DLR_SMALL_THREADS, sm, c->st>>>(a);
     CK(cudaGetLastError());
 }
@@ -514,7 +520,8 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
 // Electric field from rho = A * p (p holds the minus sign and the quadrature weight): eqs. (12)/(13) + Poisson
 // (PAPER.md:180-190):  r2c -> FFT2 -> FFT3, E_hat = -i kt phi_hat, back -> E (3 x N_x real).
 // p = scale * S vec (S != nullptr; vec has element stride vstride) or scale * vec is formed inside the first pass.
-void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int vstride, double scale) {
+void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int vstride, double scale, double* Eout = nullptr) {
+    if (Eout == nullptr) Eout = c->E;
     const HostGrid& hg = c->gx;
     D1Args a = d1args(c, hg);
     a.in_real = A; a.out_cplx = c->Eh; a.rho_S = S; a.rho_vec = vec; a.rho_stride = vstride; a.rho_scale = scale;
@@ -526,7 +533,7 @@ void field(dlr_ctx* c, const double* A, const double* S, const double* vec, int 
     CK((launch_d3<1, 3, D3_POISSON, false>(b, c->st)));
     run_d2(c, hg, c->Eh, 3, true);
     D1Args e = d1args(c, hg);
-    e.T = hg.T1s; e.in_cplx = c->Eh; e.out_real = c->E;
+    e.T = hg.T1s; e.in_cplx = c->Eh; e.out_real = Eout;
     CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
 }
 
@@ -667,7 +674,10 @@ void issue_step(dlr_ctx* c, double tau) {
         c->bytes_step = c->bytes_acc;
         return;
     }
-    lpred_sums(c, tp);                           // only rho(L1) = L1^T omega_v is needed (eq. (13)): no flow, see k_lpred_sums
+    // only rho(L1) = L1^T omega_v is needed (eq. (13)): no flow, see k_lpred_sums.  DLR_FLAG_PREDICTOR_L_FLOW runs the
+    // Lie flow of Algorithm 1 line 9 literally instead (A/B check of the marginal-based shortcut)
+    if (c->cfg.flags & DLR_FLAG_PREDICTOR_L_FLOW) flow(c, gv, c->V, true, 1, true);
+    else lpred_sums(c, tp);
     phase_mark(c, "L step (predictor)");
     // ---- Algorithm 2, line 2: E^{1/2} from X1 and L1, eq. (13)
     field_fork(c, Xp, nullptr, c->zsum, 1, -gv.g.h3);
@@ -743,6 +753,36 @@ const char* dlr_strerror(int code) {
 
 const char* dlr_last_cuda_error(dlr_ctx* c) { return c ? c->last_err_msg.c_str() : ""; }
 
+int dlr_clear_error(dlr_ctx* c) {
+    if (!c) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
+    cudaGetLastError();                        // drop a non-sticky runtime error, if any
+    c->last_err = cudaSuccess;
+    c->last_err_msg.clear();
+    c->field_pending = false;
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }      // a failed capture may have left it stale
+    c->has_state = false;                      // the state may be half-updated: dlr_set_initial must follow
+    c->vh_valid = false;
+    return DLR_OK;
+}
+
+// shared-memory opt-in of every kernel this context may launch, on the current (= the context's) device
+static cudaError_t configure_kernels(dlr_ctx* c) {
+    cudaError_t e = c->ops->configure();
+#define OPTIN(...) if (e == cudaSuccess) e = dlr_optin_smem(__VA_ARGS__)
+    OPTIN(k_d2<true>);
+    OPTIN(k_d2<false>);
+    OPTIN(k_d3<1, 3, D3_POISSON, false>);
+    OPTIN(k_d3<3, 3, D3_FWD_STORE, false>);
+    OPTIN(k_d3<3, 3, D3_INV_ONLY, false>);
+    OPTIN(k_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>);
+    OPTIN(k_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>);
+    OPTIN(k_post);
+    OPTIN(k_lpred_sums);
+#undef OPTIN
+    return e;
+}
+
 static void init_grids(dlr_ctx* c) {
     setup_grid(c->gx, c->cfg.n_x[0], c->cfg.x_lo[0], c->cfg.x_hi[0], c->R);
     setup_grid(c->gv, c->cfg.n_v[0], c->cfg.v_lo[0], c->cfg.v_hi[0], c->R);
@@ -773,6 +813,14 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev == 0) { delete c; return DLR_ERR_CUDA; }
+    // the context lives on the device that owns the workspace, whatever the caller's current device is
+    cudaPointerAttributes pa;
+    e = cudaPointerGetAttributes(&pa, d_workspace);
+    if (e != cudaSuccess || pa.type != cudaMemoryTypeDevice) { cudaGetLastError(); delete c; return DLR_ERR_WORKSPACE; }
+    c->dev = pa.device;
+    DevGuard guard(c->dev);
+    e = configure_kernels(c);
+    if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
     e = cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
@@ -793,6 +841,7 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
 
 void dlr_destroy(dlr_ctx* c) {
     if (!c) return;
+    DevGuard guard(c->dev);
     if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->cap_st) cudaStreamDestroy(c->cap_st);
     if (c->side) cudaStreamDestroy(c->side);
@@ -828,6 +877,7 @@ static int gram_check(dlr_ctx* c, const HostGrid& hg, const double* A) {
 
 int dlr_set_initial(dlr_ctx* c, const double* X, const double* S, const double* V, int on_device) {
     if (!c || !X || !S || !V) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
     const cudaMemcpyKind k = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     const int R = c->R;
     cudaError_t e = cudaMemcpyAsync(c->X, X, (size_t)c->gx.g.N * R * sizeof(double), k, c->st);
@@ -847,6 +897,7 @@ int dlr_set_initial(dlr_ctx* c, const double* X, const double* S, const double* 
 
 int dlr_step(dlr_ctx* c, double tau) {
     if (!c) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
     if (!c->has_state) return DLR_ERR_NO_STATE;
     if (c->last_err != cudaSuccess) return DLR_ERR_CUDA;
     if (c->profiling || !c->vh_valid) {
@@ -910,6 +961,7 @@ int dlr_set_profiling(dlr_ctx* c, int on) {
 
 int dlr_get_phase_times(dlr_ctx* c, int cap, float* ms, const char** names) {
     if (!c) return 0;
+    DevGuard guard(c->dev);
     cudaStreamSynchronize(c->st);
     int n = 0;
     for (size_t i = 1; i < c->phases.size() && n < cap; i++, n++) {
@@ -924,6 +976,7 @@ int dlr_get_phase_times(dlr_ctx* c, int cap, float* ms, const char** names) {
 int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* probe_ix, const int64_t* probe_iv,
                 double* f_probe) {
     if (!c || !out) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
     if (!c->has_state) return DLR_ERR_NO_STATE;
     if (n_probe < 0 || n_probe > c->probe_cap || (n_probe > 0 && (!probe_ix || !probe_iv || !f_probe))) return DLR_ERR_INVALID;
     const int R = c->R;
@@ -934,9 +987,9 @@ int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* prob
     k_colmoments_sum<<<1, 256, 0, c->st>>>(c->mxp, c->mvp, R, c->mx, c->mv);
     CK(cudaGetLastError());
     // electric energy: E from eq. (12) on the current factors.  rho_tilde = h_v^3 V^T 1 = h_v^3 * mv[:,0]
-    // (uses the scratch field buffers; the step does not depend on them across steps)
-    field(c, c->X, c->S, c->mv, 5, -c->gv.g.h3);
-    k_sumsq<<<DLR_ECH, 256, 0, c->st>>>(c->E, 3 * c->gx.g.N, c->esum);
+    // (into the diagnostics' own field buffer: dlr_get_field keeps returning the field dlr_step used last)
+    field(c, c->X, c->S, c->mv, 5, -c->gv.g.h3, c->Em);
+    k_sumsq<<<DLR_ECH, 256, 0, c->st>>>(c->Em, 3 * c->gx.g.N, c->esum);
     CK(cudaGetLastError());
     k_moments_final<<<1, 32, 0, c->st>>>(c->mx, c->mv, c->S, R, c->gx.g.h3, c->gv.g.h3, c->esum, c->mres);
     CK(cudaGetLastError());
@@ -962,11 +1015,14 @@ int dlr_moments(dlr_ctx* c, dlr_moments_t* out, int n_probe, const int64_t* prob
     out->nonfinite = res[6] != 0.0;
     out->electric_energy = 0.5 * c->gx.g.h3 * res[7];
     out->qr_fallbacks = st[0];
+    out->qr_third_stage = st[2];
+    out->eig_unconverged = st[3];
     return DLR_OK;
 }
 
 int dlr_get_factors(dlr_ctx* c, double* X, double* S, double* V, int on_device) {
     if (!c) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
     if (!c->has_state) return DLR_ERR_NO_STATE;
     const cudaMemcpyKind k = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     const int R = c->R;
@@ -981,6 +1037,7 @@ int dlr_get_factors(dlr_ctx* c, double* X, double* S, double* V, int on_device) 
 
 int dlr_get_field(dlr_ctx* c, double* E, int on_device) {
     if (!c || !E) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
     cudaError_t e = cudaMemcpyAsync(E, c->E, (size_t)3 * c->gx.g.N * sizeof(double),
                                     on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
@@ -989,6 +1046,7 @@ int dlr_get_field(dlr_ctx* c, double* E, int on_device) {
 
 int dlr_test_fft_roundtrip(dlr_ctx* c, int which, int ncols, const double* d_in, double* d_out, double* d_spec) {
     if (!c || !d_in || !d_out || !d_spec) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
     if (ncols != 3) return DLR_ERR_UNSUPPORTED;
     const HostGrid& hg = which ? c->gv : c->gx;
     if (hg.g.NC > c->gx.g.NC) return DLR_ERR_UNSUPPORTED;      // the scratch spectrum is sized for the x grid
@@ -1014,6 +1072,69 @@ int dlr_test_fft_roundtrip(dlr_ctx* c, int which, int ncols, const double* d_in,
     CK((launch_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>(e, c->st)));
     er = cudaStreamSynchronize(c->st);
     if (er != cudaSuccess) return fail(c, er, "fft inverse");
+    return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;
+}
+
+int dlr_test_chol_decide(dlr_ctx* c, const double* gram_upper, int* third_stage_needed) {
+    if (!c || !gram_upper || !third_stage_needed) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
+    const int R = c->R, P = R * (R + 1) / 2;
+    int st_before[4], st_after[4];
+    cudaError_t e = cudaMemcpyAsync(c->gram2, gram_upper, P * sizeof(double), cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st_before, c->status, sizeof(st_before), cudaMemcpyDeviceToHost, c->st);
+    if (e != cudaSuccess) return fail(c, e, "dlr_test_chol_decide");
+    // stage 1 of the CholeskyQR of a factor whose once-orthogonalised Gram matrix is gram_upper (one partial row)
+    k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->gram2, 1, R, 1, 0, 0.0, 1.0, 1.0, 0, c->apply, c->Rtot, c->Sp,
+                                                      c->status, c->status + 1);
+    CK(cudaGetLastError());
+    e = cudaMemcpyAsync(st_after, c->status, sizeof(st_after), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->status, st_before, sizeof(st_before), cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) return fail(c, e, "dlr_test_chol_decide");
+    *third_stage_needed = st_after[1] ? 0 : 1;
+    return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;
+}
+
+int dlr_test_dir_pass(dlr_ctx* c, int which, int kind, const double* d_in, double* d_out, const double* min_,
+                      const double* mout, const double* tabs, const double* Q, const double* d_E) {
+    if (!c || !d_in || !d_out || !tabs || kind < 0 || kind > 3) return DLR_ERR_INVALID;
+    if (kind >= 2 && (!Q || (which == 0 && !d_E))) return DLR_ERR_INVALID;
+    DevGuard guard(c->dev);
+    const HostGrid& hg = which ? c->gv : c->gx;
+    const int R = c->R, RR = R * R, n = hg.g.n, lg = hg.g.log2n;
+    const int ntab = kind < 2 ? 1 : 4;
+    // tables arrive in natural wavenumber order [tab][k][column] (complex); the kernels index them by stored position
+    std::vector<double2> t((size_t)ntab * n * R);
+    const double2* src = (const double2*)tabs;
+    for (int q = 0; q < ntab; q++)
+        for (int e = 0; e < n; e++)
+            for (int j = 0; j < R; j++) t[((size_t)q * n + e) * R + j] = src[((size_t)q * n + brev_host(e, lg)) * R + j];
+    double2* dst[4] = {kind < 2 ? c->ft.p.ph1 : c->ft.p.ez, c->ft.p.f1, c->ft.p.f2a, c->ft.p.f2b};
+    cudaError_t e = cudaSuccess;
+    for (int q = 0; q < ntab && e == cudaSuccess; q++)
+        e = cudaMemcpyAsync(dst[q], t.data() + (size_t)q * n * R, (size_t)n * R * sizeof(double2), cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess && min_) e = cudaMemcpyAsync(c->ft.p.mats, min_, RR * sizeof(double), cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess && mout) e = cudaMemcpyAsync(c->ft.p.mats + RR, mout, RR * sizeof(double), cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess && Q) e = cudaMemcpyAsync(c->ft.p.Q, Q, 3 * RR * sizeof(double), cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);          // the staging vector goes out of scope below
+    if (e != cudaSuccess) return fail(c, e, "dlr_test_dir_pass");
+    DirArgs a = dirargs(c, hg);
+    a.in = d_in; a.out = d_out; a.store = 1;
+    a.min_ = min_ ? c->ft.p.mats : nullptr; a.mout = mout ? c->ft.p.mats + RR : nullptr;
+    if (kind < 2) {
+        a.L = hg.Lx; a.ph = c->ft.p.ph1;
+        if (kind == 1) { a.threads = hg.thrx2; a.min_ = a.mout = nullptr; }
+        CK(c->ops->dir[kind == 0 ? VD_EXACT1 : VD_EXACT2](a, c->st));
+    } else {
+        a.threads = hg.thre; a.L = hg.Le; a.E = d_E; a.Q = c->ft.p.Q;
+        a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1; a.f2a = c->ft.p.f2a; a.f2b = c->ft.p.f2b;
+        const int v = kind == 2 ? (which ? VD_ETD1_V : VD_ETD1_E) : (which ? VD_ETD2_V : VD_ETD2_E);
+        CK(c->ops->dir[v](a, c->st));
+    }
+    e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) return fail(c, e, "dlr_test_dir_pass");
+    c->vh_valid = false;                 // the flow tables were overwritten: the next step rebuilds everything
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
     return c->last_err == cudaSuccess ? DLR_OK : DLR_ERR_CUDA;
 }
 

@@ -22,6 +22,24 @@ struct GridDev {
     const double2* tw;       // [n/2] exp(-2 pi i k / n)
 };
 
+// Opt a kernel in to the whole dynamic shared memory of an SM of the CURRENT device.  cudaFuncSetAttribute is state
+// of (function, device), not of a context: every dlr_create does this once for all kernels it may launch (idempotent,
+// same value from every context and thread), so the library keeps no process-wide "already configured" flags.
+template <class K>
+inline cudaError_t dlr_optin_smem(K kern) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    int dev = 0, optin = 0;
+    e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    return e;
+}
+
 // ---------------------------------------------------------------- complex helpers
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }

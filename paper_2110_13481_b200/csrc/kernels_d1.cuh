@@ -222,14 +222,6 @@ inline cudaError_t launch_d1(const D1Args& a, cudaStream_t st) {
     constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : 0;
     auto kern = k_d1<RIN, ROUT, IN_MODE, OP, GRAM, OUT_MODE>;
     const size_t sm = d1_smem_bytes(a.g.n, RMAX, a.T, false, (NMAT + 1) & ~1);
-    static size_t configured = 0;
-    if (sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
     const unsigned grid = (unsigned)(((long long)a.g.n * a.g.n) / a.T);
     kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
     return cudaGetLastError();

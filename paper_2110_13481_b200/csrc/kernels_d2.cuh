@@ -68,14 +68,6 @@ template <bool INV>
 inline cudaError_t launch_d2(const D2Args& a, cudaStream_t st) {
     auto kern = k_d2<INV>;
     const size_t sm = d2_smem_bytes(a.g.n, a.T2, a.NB);
-    static size_t configured = 0;
-    if (sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
     const long long nslab = (long long)a.ncols * a.g.n;
     const unsigned grid = (unsigned)(a.nchunks * ((nslab + a.NB - 1) / a.NB));
     kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);

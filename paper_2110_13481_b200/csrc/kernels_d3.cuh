@@ -92,14 +92,6 @@ inline cudaError_t launch_d3(const D3Args& a, cudaStream_t st) {
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
     auto kern = k_d3<RIN, ROUT, FOP, UNUSED>;
     const size_t sm = d3_smem_bytes(a.g.n, RMAX, a.T, 0);
-    static size_t configured = 0;
-    if (sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
     const long long plane = (long long)a.g.nh * a.g.n;
     const unsigned grid = (unsigned)((plane + a.T - 1) / a.T);
     kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);

@@ -495,14 +495,6 @@ inline cudaError_t launch_dir(const DirArgs& a, cudaStream_t st) {
     constexpr bool ETD = (DOP == DOP_ETD1 || DOP == DOP_ETD2);
     auto kern = k_dir<R, DIR, DOP, DW>;
     const size_t sm = dir_smem_bytes(a.g.n, R, a.L, ETD ? 2 : 1, ETD ? 5 : 2, DW == DW_E);
-    static size_t configured = 0;
-    if (sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
     kern<<<(unsigned)dir_tiles(a.g.n, a.L), a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
     return cudaGetLastError();
 }

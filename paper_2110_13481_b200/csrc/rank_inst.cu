@@ -9,11 +9,33 @@
 
 namespace {
 constexpr int R = DLR_RANK;
+
+cudaError_t configure_rank() {
+    cudaError_t e = cudaSuccess;
+#define OPTIN(...) if (e == cudaSuccess) e = dlr_optin_smem(__VA_ARGS__)
+    OPTIN(k_d1<R, R, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_PLAIN, D1_OUT_REAL>);
+    OPTIN(k_d1<R, R, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_NONE, D1_OUT_REAL>);
+    OPTIN(k_d1<R, R, D1_IN_REAL, D1_OP_NONE, D1_GRAM_PLAIN, D1_OUT_NONE>);
+    OPTIN(k_d1<R, 1, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_NONE, D1_OUT_CPLX>);
+    OPTIN(k_dir<R, 1, DOP_EXACT, DW_NONE>);
+    OPTIN(k_dir<R, 2, DOP_EXACT, DW_NONE>);
+    OPTIN(k_dir<R, 3, DOP_ETD1, DW_E>);
+    OPTIN(k_dir<R, 3, DOP_ETD1, DW_V>);
+    OPTIN(k_dir<R, 3, DOP_ETD2, DW_E>);
+    OPTIN(k_dir<R, 3, DOP_ETD2, DW_V>);
+    OPTIN(k_dir<R, 1, DOP_COEFF, DW_V>);
+    OPTIN(k_dir<R, 1, DOP_COEFF, DW_E>);
+    OPTIN(k_dir<R, 2, DOP_COEFF, DW_NONE>);
+    OPTIN(k_dir<R, 3, DOP_COEFF, DW_NONE>);
+#undef OPTIN
+    return e;
 }
+}  // namespace
 
 extern "C" const RankOps* CAT(dlr_rank_ops_, DLR_RANK)() {
     static const RankOps ops = {
         R,
+        configure_rank,
         {
             launch_d1<R, R, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_PLAIN, D1_OUT_REAL>,
             launch_d1<R, R, D1_IN_REAL, D1_OP_MATVEC, D1_GRAM_NONE, D1_OUT_REAL>,

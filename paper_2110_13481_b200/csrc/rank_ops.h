@@ -31,6 +31,7 @@ enum {
 
 struct RankOps {
     int R;
+    cudaError_t (*configure)();      // shared-memory opt-in of every kernel below on the current device (dlr_create)
     cudaError_t (*d1[V1_COUNT])(const D1Args&, cudaStream_t);
     cudaError_t (*dir[VD_COUNT])(const DirArgs&, cudaStream_t);
 };

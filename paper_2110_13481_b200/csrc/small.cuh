@@ -63,7 +63,7 @@ __device__ __forceinline__ void cta_reduce_rows(const double* __restrict__ parti
 #define DLR_EIG_THREADS 256
 __global__ void __launch_bounds__(DLR_EIG_THREADS)
 k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double h3, double* M1, double* colsum,
-             double* Tout, double* lam, int warm) {
+             double* Tout, double* lam, int warm, int* status) {
     __shared__ double As[2][DLR_RMAXS][DLR_RMAXS + 1], Ts[2][DLR_RMAXS][DLR_RMAXS + 1];
     __shared__ double red[DLR_RMAXS * (DLR_RMAXS + 1) / 2], tmp[DLR_EIG_THREADS];
     __shared__ double alpha[DLR_RMAXS], beta[DLR_RMAXS], sq[DLR_RMAXS];
@@ -120,6 +120,7 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
     const double nrm2 = s_nrm2;
     const int m = R + (R & 1), half = m >> 1;
     int cur = 0;
+    bool converged = false;
     for (int sweep = 0; sweep < 40; sweep++) {
         double myoff = 0.0;                                     // sum of apq^2 met by this thread's pairs
         for (int r = 0; r < m - 1; r++) {
@@ -174,8 +175,9 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
             s_off2 = o;
         }
         __syncthreads();
-        if (s_off2 <= 1e-32 * nrm2) break;                     // off-diagonal norm met in this sweep <= 1e-16 ||A||_F
+        if (s_off2 <= 1e-32 * nrm2) { converged = true; break; }   // off-diagonal norm met in this sweep <= 1e-16 ||A||_F
     }
+    if (!converged && tid == 0) atomicAdd(status + 3, 1);      // sweep cap hit: reported as dlr_moments_t.eig_unconverged
     if (warm) {
         // one Newton-Schulz step T <- T (3 I - T^T T) / 2 keeps the accumulated T orthogonal to rounding level no matter
         // how many steps it has been carried along
@@ -439,10 +441,13 @@ __global__ void __launch_bounds__(DLR_SMALL_THREADS) k_colsum_reduce(const doubl
 //   apply[ci][co] : matrix for the next A*Mat pass (= D U^-1, times out_scale on the last stage)
 //   Rtot (row-major, upper triangular) accumulates R_stage * Rtot with R_stage = U D^-1.
 //   On the last stage the coupling matrix is written: Sout column-major = Rtot*s_scale (transS=0) or its transpose.
-//   Adaptive third stage: stage 1 holds the Gram matrix of the once-orthogonalised factor; if its largest scaled
-//   off-diagonal entry is < 0.1 the factor after this stage is orthonormal to rounding level (CholeskyQR2 suffices for
+//   Adaptive third stage: stage 1 holds the Gram matrix G of the once-orthogonalised factor, scaled to unit diagonal.
+//   If the Frobenius norm of its off-diagonal part is < 0.5 then ||G - I||_2 < 0.5, i.e. kappa(G) < 3 for every rank
+//   (a sufficient criterion, unlike a bound on the largest entry: a unit-diagonal Gram with all off-diagonals -1/19 is
+//   singular at r = 20), the factor after this stage is orthonormal to rounding level (CholeskyQR2 suffices for
 //   kappa(A)^2 u < 1), so stage 1 acts as the last stage and sets qrflag[0] = 1: the stage-1 A*Mat pass then writes
-//   the basis directly and the stage-2 kernels return at once.  Stage 0 clears the flag.
+//   the basis directly and the stage-2 kernels return at once.  Stage 0 clears the flag.  status[2] counts the QRs that
+//   needed the third stage.
 __global__ void __launch_bounds__(DLR_SMALL_THREADS)
 k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, double shift, double out_scale,
              double s_scale, int transS, double* apply, double* Rtot, double* Sout, int* status, int* qrflag) {
@@ -475,17 +480,17 @@ k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, dou
     }
     __syncthreads();
     __shared__ int s_skip;
-    if (threadIdx.x < 32) {                                     // largest off-diagonal entry of the scaled Gram matrix
-        double mx = 0.0;
+    if (threadIdx.x < 32) {                                     // squared Frobenius norm of the off-diagonal part
+        double f2 = 0.0;
         for (int idx = threadIdx.x; idx < RR; idx += 32) {
             const int i = idx / R, j = idx - i * R;
-            if (i != j) mx = fmax(mx, fabs(G[i][j]));
+            if (i != j) f2 = fma(G[i][j], G[i][j], f2);
         }
-        for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        f2 = warp_sum(f2);
         if (threadIdx.x == 0) {
-            s_skip = (stage == 1 && mx < 0.1) ? 1 : 0;
+            s_skip = (stage == 1 && f2 < 0.25) ? 1 : 0;          // NaN compares false: no skip
             if (stage == 0) qrflag[0] = 0;
-            if (stage == 1) qrflag[0] = s_skip;
+            if (stage == 1) { qrflag[0] = s_skip; if (!s_skip) atomicAdd(status + 2, 1); }
         }
     }
     __syncthreads();

@@ -28,7 +28,8 @@ class dlr_config(ctypes.Structure):
 class dlr_moments_t(ctypes.Structure):
     _fields_ = [("mass", ctypes.c_double), ("momentum", ctypes.c_double * 3), ("kinetic_energy", ctypes.c_double),
                 ("electric_energy", ctypes.c_double), ("s_fro", ctypes.c_double),
-                ("qr_fallbacks", ctypes.c_int32), ("nonfinite", ctypes.c_int32)]
+                ("qr_fallbacks", ctypes.c_int32), ("nonfinite", ctypes.c_int32),
+                ("qr_third_stage", ctypes.c_int32), ("eig_unconverged", ctypes.c_int32)]
 
 
 _lib = None
@@ -57,12 +58,15 @@ def lib():
         L.dlr_bytes_per_step.argtypes = [vp]
         L.dlr_bytes_per_step.restype = ctypes.c_double
         L.dlr_test_fft_roundtrip.argtypes = [vp, ip, ip, vp, vp, vp]
+        L.dlr_test_dir_pass.argtypes = [vp, ip, ip, vp, vp, vp, vp, vp, vp, vp]
+        L.dlr_test_chol_decide.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_int)]
         L.dlr_destroy.argtypes = [vp]
         L.dlr_destroy.restype = None
         L.dlr_strerror.argtypes = [ip]
         L.dlr_strerror.restype = ctypes.c_char_p
         L.dlr_last_cuda_error.argtypes = [vp]
         L.dlr_last_cuda_error.restype = ctypes.c_char_p
+        L.dlr_clear_error.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -73,18 +77,22 @@ class DlrError(RuntimeError):
         super().__init__(f"{where}: {ERRORS.get(code, code)} ({lib().dlr_strerror(code).decode()}) {detail}")
 
 
-def make_config(n_x, n_v, x_lo, x_hi, v_lo, v_hi, rank, order=2, e_scale=1.0):
+FLAG_PREDICTOR_L_FLOW = 1
+
+
+def make_config(n_x, n_v, x_lo, x_hi, v_lo, v_hi, rank, order=2, e_scale=1.0, flags=0):
     c = dlr_config()
     for d in range(3):
         c.n_x[d], c.n_v[d] = n_x, n_v
         c.x_lo[d], c.x_hi[d], c.v_lo[d], c.v_hi[d] = x_lo, x_hi, v_lo, v_hi
-    c.rank, c.order, c.e_scale, c.flags = rank, order, e_scale, 0
+    c.rank, c.order, c.e_scale, c.flags = rank, order, e_scale, flags
     return c
 
 
-def config_from_inputs(cfg, order=2, e_scale=1.0):
+def config_from_inputs(cfg, order=2, e_scale=1.0, flags=0):
     """dlr_config from a dict of paper_2110_13481_b200.inputs.make_config"""
-    return make_config(cfg["n_x"], cfg["n_v"], cfg["x_lo"], cfg["x_hi"], cfg["v_lo"], cfg["v_hi"], cfg["r"], order, e_scale)
+    return make_config(cfg["n_x"], cfg["n_v"], cfg["x_lo"], cfg["x_hi"], cfg["v_lo"], cfg["v_hi"], cfg["r"], order, e_scale,
+                       flags)
 
 
 def dlr_workspace_bytes(cfg):
@@ -161,7 +169,7 @@ class Dlr:
         self._check(lib().dlr_moments(self.h, ctypes.byref(m), npb, _ptr(ix), _ptr(iv), _ptr(f)), "dlr_moments")
         out = {"mass": m.mass, "momentum": list(m.momentum), "kinetic_energy": m.kinetic_energy,
                "electric_energy": m.electric_energy, "s_fro": m.s_fro, "qr_fallbacks": m.qr_fallbacks,
-               "nonfinite": m.nonfinite}
+               "nonfinite": m.nonfinite, "qr_third_stage": m.qr_third_stage, "eig_unconverged": m.eig_unconverged}
         return (out, f) if npb else out
 
     def get_factors(self, out=None):
@@ -181,6 +189,9 @@ class Dlr:
         E = np.empty((3, self.Nx))
         self._check(lib().dlr_get_field(self.h, _ptr(E), 0), "dlr_get_field")
         return E
+
+    def clear_error(self):
+        self._check(lib().dlr_clear_error(self.h), "dlr_clear_error")
 
     def set_profiling(self, on):
         self._check(lib().dlr_set_profiling(self.h, int(on)), "dlr_set_profiling")
@@ -211,6 +222,28 @@ class Dlr:
                                                  d_spec.data_ptr()), "dlr_test_fft_roundtrip")
         spec = d_spec.cpu().numpy().view(np.complex128).reshape(ncols, n, n, n // 2 + 1)
         return np.asfortranarray(d_out.cpu().numpy().T), spec
+
+    def test_dir_pass(self, which, kind, A, tabs, min_=None, mout=None, Q=None, E=None):
+        """one directional pass (include/dlr.h): A (N, r) Fortran-order numpy -> result of the same shape;
+        tabs: complex (ntab, n, r) in natural DFT order; min_, mout (r, r) [cin][cout]; Q (3, r, r); E (3, N_x)"""
+        torch = self.torch
+        d_in = torch.from_numpy(np.ascontiguousarray(A.T)).to(self.device)
+        d_out = torch.empty_like(d_in)
+        d_E = None if E is None else torch.from_numpy(np.ascontiguousarray(E)).to(self.device)
+        c = lambda a, dt=np.float64: None if a is None else np.ascontiguousarray(a, dtype=dt)
+        tabs, min_, mout, Q = c(tabs, np.complex128), c(min_), c(mout), c(Q)
+        self._check(lib().dlr_test_dir_pass(self.h, which, kind, d_in.data_ptr(), d_out.data_ptr(), _ptr(min_), _ptr(mout),
+                                            _ptr(tabs), _ptr(Q), _ptr(d_E)), "dlr_test_dir_pass")
+        return np.asfortranarray(d_out.cpu().numpy().T)
+
+    def test_chol_decide(self, G):
+        """does the adaptive CholeskyQR ask for a third stage, given the (r, r) Gram matrix of the once-orthogonalised
+        factor?"""
+        r = self.r
+        up = np.ascontiguousarray([G[i, j] for i in range(r) for j in range(i, r)], dtype=np.float64)
+        out = ctypes.c_int(0)
+        self._check(lib().dlr_test_chol_decide(self.h, _ptr(up), ctypes.byref(out)), "dlr_test_chol_decide")
+        return bool(out.value)
 
     def close(self):
         if getattr(self, "h", None):

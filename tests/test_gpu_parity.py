@@ -37,16 +37,16 @@ def ee_scale(hist, m):
     return hist[m]
 
 
-def make_ctx(cfg, order=2, e_scale=1.0):
+def make_ctx(cfg, order=2, e_scale=1.0, flags=0):
     from paper_2110_13481_b200 import dlr
-    return dlr.Dlr(dlr.config_from_inputs(cfg, order=order, e_scale=e_scale))
+    return dlr.Dlr(dlr.config_from_inputs(cfg, order=order, e_scale=e_scale, flags=flags))
 
 
 def check(ctx, Xo, So, Vo, gx, gv, ix, iv, tol, e_scale=1.0):
     m, f = ctx.moments(ix, iv)
     mo = O.moments(Xo, So, Vo, gx, gv, e_scale)
     fo = O.f_at(Xo, So, Vo, ix, iv)
-    assert m["qr_fallbacks"] == 0 and m["nonfinite"] == 0
+    assert m["qr_fallbacks"] == 0 and m["nonfinite"] == 0 and m["eig_unconverged"] == 0
     assert np.abs(f - fo).max() <= tol * np.abs(fo).max()
     assert rel(m["mass"], mo["mass"]) <= tol
     if e_scale:
@@ -139,18 +139,21 @@ def test_full_run_config1():
     ctx.close()
 
 
-def _golden_run(idx, max_steps=None):
-    path = os.path.join(GOLDEN, f"cfg{idx}.json")
+def _golden_run(idx, max_steps=None, name=None, **over):
+    """run the GPU path against a stored oracle run (tests/golden/, written by make_golden.py from oracle/ alone).
+    Returns (golden, GPU electric-energy history)."""
+    path = os.path.join(GOLDEN, name or f"cfg{idx}.json")
     if not os.path.exists(path):
         pytest.skip(f"{path} not generated")
     gold = json.load(open(path))
-    cfg = inputs.make_config(idx)
+    cfg = inputs.make_config(idx, **over)
     X, S, V = inputs.initial_factors(cfg)
     ix, iv = inputs.probe_indices(cfg)
     ctx = make_ctx(cfg)
     ctx.set_initial(X, S, V)
     nsteps = gold["steps"] if max_steps is None else min(max_steps, gold["steps"])
     assert gold["qr_fallbacks"] == 0
+    ee_gpu, worst_pt = [], 0.0
     for step in range(nsteps + 1):
         if step:
             ctx.step(cfg["tau"])
@@ -162,19 +165,27 @@ def _golden_run(idx, max_steps=None):
         else:
             m = ctx.moments()
         ee = gold["electric_energy"]
+        ee_gpu.append(m["electric_energy"])
+        worst_pt = max(worst_pt, rel(m["electric_energy"], ee[step]))
         assert abs(m["electric_energy"] - ee[step]) <= tol * ee_scale(ee[:nsteps + 1], step), step
         assert rel(m["mass"], gold["mass"][step]) <= tol, step
         assert rel(m["kinetic_energy"], gold["kinetic_energy"][step]) <= tol, step
-        assert m["qr_fallbacks"] == 0 and m["nonfinite"] == 0
+        assert rel(m["s_fro"], gold["s_fro"][step]) <= tol, step
+        assert m["qr_fallbacks"] == 0 and m["nonfinite"] == 0 and m["eig_unconverged"] == 0
     ctx.close()
-    return gold
+    # the literal tolerance of north_star is pointwise; reading R17 normalises strict local minima by their
+    # neighbours.  Both are reported; relative to max_t ee the history error is far below either.
+    err_hist = np.abs(np.array(ee_gpu) - np.array(ee[:nsteps + 1])).max() / max(ee[:nsteps + 1])
+    print(f"golden {os.path.basename(path)}: electric-energy history: worst pointwise rel. error {worst_pt:.2e}, "
+          f"max |diff| / max ee {err_hist:.2e}")
+    assert err_hist <= 0.1 * TOL_RUN
+    return gold, np.array(ee_gpu)
 
 
 def test_full_run_config2_golden_and_damping_rate():
     """BASELINE.json config 2 (32^3 x 32^3, r = 10, 200 steps) against tests/golden/cfg2.json (written by
     tests/golden/make_golden.py from the oracle); the GPU energy history shows the Landau rate -0.1533."""
-    gold = _golden_run(2)
-    ee = np.array(gold["electric_energy"])
+    gold, ee = _golden_run(2)                   # ee: the GPU history (it matches the oracle's to 1e-8, checked above)
     tau = gold["tau"]
     tp, lp = [], []
     for i in range(1, len(ee) - 1):
@@ -189,6 +200,69 @@ def test_config3_metric_shape_golden():
     """BASELINE.json config 3 = the metric's shape (64^3 x 64^3, r = 10, two-stream), in the launch configuration
     bench.py times, against tests/golden/cfg3.json for as many steps as the golden file holds."""
     _golden_run(3)
+
+
+@pytest.mark.parametrize("base,n_x,n_v,r", [(5, 64, 64, 20), (4, 64, 64, 15), (5, 128, 128, 20), (2, 32, 128, 10),
+                                            (4, 128, 32, 15)])
+def test_one_step_at_every_tile_shape_live_oracle(base, n_x, n_v, r):
+    """every (n, r) combination takes its own tile shape, CTA size and occupancy rule in the pass kernels
+    (api.cu::setup_grid, kernels_dir.cuh launch bounds): one step of Algorithm 2 against the oracle run live at the
+    shapes that the other tests do not reach: r = 20 and r = 15 at n = 64 (one CTA per SM at r = 20), r = 20 at
+    n = 128 (single-line tiles holding all of the shared memory, three FFT groups), mixed 32/128 grids.
+    Inputs: the recipe of BASELINE.json config `base` at these grids; r = 20 uses config 5's (band-limited rank-20
+    perturbation at 1e-6): with the rank-1 initial value of configs 1-4 the first K at r = 20, n >= 64 is rank
+    deficient to working precision, the oracle's QR replaces columns (reading R12) and the step is then defined only
+    up to that choice (measured: E^{1/2} moves by 3e-6) - parity needs a fallback-free oracle step, asserted here."""
+    cfg = inputs.make_config(base, n_x=n_x, n_v=n_v, r=r)
+    gx, gv = grids(cfg)
+    X, S, V = inputs.initial_factors(cfg)
+    ix, iv = inputs.probe_indices(cfg)
+    ctx = make_ctx(cfg)
+    ctx.set_initial(X, S, V)
+    ctx.step(cfg["tau"])
+    stats = {}
+    X, S, V = O.step_alg2(X, S, V, cfg["tau"], gx, gv, 1.0, stats)
+    assert stats.get("qr_fallbacks", 0) == 0
+    check(ctx, X, S, V, gx, gv, ix, iv, TOL_STEP)
+    ctx.close()
+
+
+@pytest.mark.parametrize("base,n_x,n_v,r", [(2, 256, 8, 10), (2, 8, 256, 10), (5, 16, 256, 20)])
+def test_one_step_at_n256_golden(base, n_x, n_v, r):
+    """the n = 256 kernel paths (three radix groups, single-line 227 KB tiles, and at r = 20 one CTA per SM with up to
+    255 registers) on the x grid and on the v grid: one step against tests/golden/shape_<n_x>_<n_v>_<r>.json, an
+    oracle step (10-20 minutes of host time each, hence stored) written by tests/golden/make_golden.py."""
+    _golden_run(base, name=f"shape_{n_x}_{n_v}_{r}.json", n_x=n_x, n_v=n_v, r=r)
+
+
+def test_config5_one_step_golden():
+    """BASELINE.json config 5 (256^3 x 256^3, r = 20, band-limited rank-20 perturbation) at FULL size, in the launch
+    configuration bench.py times: one step against tests/golden/cfg5.json (an oracle step needs ~35 GB and about an
+    hour of host time, hence stored; written by tests/golden/make_golden.py 5 1)."""
+    _golden_run(5)
+
+
+def test_predictor_L_shortcut_equals_the_flow():
+    """the predictor of Algorithm 2 takes rho(L^1) from the 1D marginals of V instead of running the L flow (DESIGN.md
+    row a7').  A/B against the literal flow (DLR_FLAG_PREDICTOR_L_FLOW) after several steps, when S has full rank and
+    the field is nonlinear (alpha = 0.5): E^{1/2} point-wise and f at the probes."""
+    from paper_2110_13481_b200 import dlr
+    for n, r, nsteps in ((64, 10, 6), (128, 15, 3)):
+        cfg = inputs.make_config(4, n_x=n, n_v=n, r=r)
+        X, S, V = inputs.initial_factors(cfg)
+        ix, iv = inputs.probe_indices(cfg)
+        res = []
+        for flags in (0, dlr.FLAG_PREDICTOR_L_FLOW):
+            ctx = make_ctx(cfg, flags=flags)
+            ctx.set_initial(X, S, V)
+            ctx.run(cfg["tau"], nsteps)
+            m, f = ctx.moments(ix, iv)
+            res.append((ctx.get_field(), f, m))
+            ctx.close()
+        (Ea, fa, ma), (Eb, fb, mb) = res
+        assert np.abs(Ea - Eb).max() <= 1e-11 * np.abs(Eb).max(), (n, r)
+        assert np.abs(fa - fb).max() <= 1e-11 * np.abs(fb).max(), (n, r)
+        assert rel(ma["electric_energy"], mb["electric_energy"]) <= 1e-11
 
 
 def test_config4_one_step():
