@@ -55,7 +55,7 @@ def measured_peak():
 # 8 N per field component).  Averages over the launches of a step where K and L flows differ.
 FAMILIES = [
     ("VD_EXACT1", "k_dir<r,1,EXACT> sub-flow 1 + column mixing", 2.0, 0.0),
-    ("VD_EXACT2", "k_dir<r,2,EXACT> sub-flow 2", 2.0, 0.0),
+    ("run_sub2", "k_sub2 sub-flow 2 (warp-autonomous units)", 2.0, 0.0),
     ("VD_ETD2", "k_dir<r,3,ETD2> third sub-flow, both ETD2RK stages", 2.0, 2.0),     # E read by 2 of 3 launches
     ("VD_ETD1", "k_dir<r,3,ETD1> third sub-flow, exponential Euler", 1.5, 1.5),      # K: 2B + E; L (sums only): B
     ("VD_COEFF1", "k_dir<r,1,COEFF> weighted Gram + Parseval", 1.0, 2.0),

@@ -12,7 +12,7 @@ LIB = os.path.join(HERE, "libdlr_b200.so")
 RANKS = (5, 8, 10, 15, 20)
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC"]
+         "-Xcompiler", "-fPIC"] + os.environ.get("DLR_NVCC_EXTRA", "").split()     # e.g. -DDLR_ENABLE_TUNE for experiments
 
 
 def _newer(target, deps):

@@ -12,6 +12,7 @@
 #include "../../include/dlr.h"
 #include "rank_ops.h"
 #include "small.cuh"
+#include "pass_sub2.cuh"
 
 extern "C" {
 const RankOps* dlr_rank_ops_5();
@@ -50,6 +51,8 @@ struct FlowTab {
     FlowTabPtrs p;
 };
 
+struct Sub2Cfg { int L, groups, wpu, ctas; };      // launch shape of the direction-2 sub-flow (pass_sub2.cuh)
+
 struct Phase {
     const char* name;
     cudaEvent_t ev;
@@ -61,6 +64,7 @@ struct dlr_ctx {
     dlr_config cfg;
     int R;
     int dev;                      // device of the workspace: every entry point runs under it (DevGuard)
+    int nsm;                      // its number of SMs (persistent grids)
     cudaStream_t st, cap_st;
     cudaStream_t side;            // side branch: the coefficient/eigen kernel overlaps the dim-2/3 passes of its transform
     cudaEvent_t ev_fork, ev_join;
@@ -71,6 +75,7 @@ struct dlr_ctx {
     double bytes_acc, bytes_step;     // algorithmic bytes of the factor-sized passes issued by the current / last step
     const RankOps* ops;
     HostGrid gx, gv;
+    Sub2Cfg s2x, s2v;
     // big buffers
     double *X, *X1, *V, *S, *Sp;     // X1: the predictor basis of Algorithm 2 (X itself stays X0 until the first K step)
     double2* Eh;
@@ -289,6 +294,7 @@ size_t carve(dlr_ctx* c, char* base) {
         hg->g.kt2p = t ? t + 2 * nh : nullptr; hg->g.ksq2p = t ? t + 2 * nh + n : nullptr;
         double2* tw = cv.take<double2>(n / 2);
         hg->g.tw = tw;
+        hg->g.wtab = cv.take<double2>((size_t)wf_plan(hg->g.log2n).tlen + 1);
     }
     return align_up(cv.off, 256);
 }
@@ -359,6 +365,10 @@ cudaError_t upload_tables(dlr_ctx* c, HostGrid& hg, double lo, double hi) {
         tw[k] = make_double2((double)cosl(a), (double)sinl(a));
     }
     e = cudaMemcpyAsync((void*)hg.g.tw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice, c->st);
+    if (e != cudaSuccess) return e;
+    std::vector<double2> wt((size_t)wf_plan(lg).tlen + 1);
+    wf_host_tables(lg, wt.data());
+    e = cudaMemcpyAsync((void*)hg.g.wtab, wt.data(), wt.size() * sizeof(double2), cudaMemcpyHostToDevice, c->st);
     if (e != cudaSuccess) return e;
     return cudaStreamSynchronize(c->st);
 }
@@ -435,6 +445,31 @@ DirArgs dirargs(dlr_ctx* c, const HostGrid& hg) {
     return a;
 }
 int dir_blocks(const HostGrid& hg, int L) { return dir_tiles(hg.g.n, L); }
+
+// sub-flow along direction 2 (pass_sub2.cuh): one warp per unit, as many resident warps as the SM holds
+void setup_sub2(dlr_ctx* c, const HostGrid& hg, Sub2Cfg& sc) {
+    // measured at 64^3, r = 10 (B200): 128-byte segments (L = 8) and small CTAs (4 groups) win: 14.4 us per pass
+    // against 18.4 (L = 4, 8 warps) and 19.1 for the CTA-tile kernel of round 1.  Larger n: keep a unit near 10 KB
+    // per warp (L = 4, and two warps per unit at n = 256)
+    const int n = hg.g.n, M = n / 2;
+    sc.L = n <= 64 ? std::min(M, 8) : 4;
+    sc.wpu = n >= 256 ? 2 : 1;
+    sc.groups = 4;
+    { const int l = tune("s2l", 0); if (is_pow2(l) && l <= M) sc.L = l; }
+    { const int w = tune("s2w", 0); if (w >= 1 && w <= 8) sc.groups = w; }
+    { const int w = tune("s2u", 0); if (w == 1 || w == 2 || w == 4) sc.wpu = w; }
+    while (sc.groups > 1 && sub2_smem_bytes(n, sc.L, sc.groups) > SMEM_MAX - 1024) sc.groups /= 2;
+    const int per_sm = sub2_occupancy(hg.g.log2n, sc.groups * sc.wpu, sub2_smem_bytes(n, sc.L, sc.groups));
+    const int units = n * (M / sc.L);
+    const int want = (c->nsm * per_sm + c->R - 1) / c->R;                 // CTAs per column to fill the device once
+    sc.ctas = std::max(1, std::min(want, (units + sc.groups - 1) / sc.groups));
+}
+cudaError_t run_sub2(dlr_ctx* c, const HostGrid& hg, const double* in, double* out, const double2* ph) {
+    const Sub2Cfg& sc = (&hg == &c->gx) ? c->s2x : c->s2v;
+    Sub2Args a;
+    a.g = hg.g; a.in = in; a.out = out; a.ph = ph; a.R = c->R; a.L = sc.L; a.wpu = sc.wpu;
+    return launch_sub2(a, sc.groups, sc.ctas, c->st);
+}
 
 // Coefficient set of a factor A (N x r, real):  kind = 1: C coefficients (weights v_i, + rho_tilde);  2: D coefficients
 // (weights E_i).  Three read-only passes, one per direction: the first also accumulates the real-space weighted Gram
@@ -596,9 +631,8 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     CK(ops->dir[VD_EXACT1](a, c->st));
     c->bytes_acc += (order == 1 ? (zero_only ? 5.0 : 6.0) : 10.0) * fac_bytes(c, hg) + (is_L ? 0.0 : 24.0 * (double)hg.g.N);
     // sub-flow 2
-    a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2; a.threads = hg.thrx2;
-    CK(ops->dir[VD_EXACT2](a, c->st));
-    a.threads = hg.thrx;
+    a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
+    CK(run_sub2(c, hg, c->W, c->W, c->ft.p.ph2));
     // sub-flow 3 in the eigenbasis of direction 3 (the first pass of a K flow that reads the electric field)
     field_join(c);
     DirArgs e = dirargs(c, hg);
@@ -617,9 +651,7 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
     }
     e.mout = mats + 5 * RR; e.store = 1; e.out = c->W;          // T3^T T2
     CK(ops->dir[is_L ? VD_ETD2_V : VD_ETD2_E](e, c->st));
-    a.threads = hg.thrx2;
-    CK(ops->dir[VD_EXACT2](a, c->st));                           // sub-flow 2, second half
-    a.threads = hg.thrx;
+    CK(run_sub2(c, hg, c->W, c->W, c->ft.p.ph2));                // sub-flow 2, second half
     a.out = c->KL; a.min_ = mats + 6 * RR; a.mout = mats + 7 * RR; a.ph = c->ft.p.ph1; a.gram = c->partial;
     CK(ops->dir[VD_EXACT1](a, c->st));                           // sub-flow 1, second half, + Gram of the result
     return dir_blocks(hg, hg.Lx);
@@ -778,6 +810,7 @@ static cudaError_t configure_kernels(dlr_ctx* c) {
     OPTIN(k_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>);
     OPTIN(k_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>);
     OPTIN(k_post);
+    if (e == cudaSuccess) e = configure_sub2();
     OPTIN(k_lpred_sums);
 #undef OPTIN
     return e;
@@ -819,8 +852,11 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e != cudaSuccess || pa.type != cudaMemoryTypeDevice) { cudaGetLastError(); delete c; return DLR_ERR_WORKSPACE; }
     c->dev = pa.device;
     DevGuard guard(c->dev);
+    if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->dev) != cudaSuccess || c->nsm < 1) c->nsm = 148;
     e = configure_kernels(c);
     if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
+    setup_sub2(c, c->gx, c->s2x);
+    setup_sub2(c, c->gv, c->s2v);
     e = cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
@@ -1123,8 +1159,8 @@ int dlr_test_dir_pass(dlr_ctx* c, int which, int kind, const double* d_in, doubl
     a.min_ = min_ ? c->ft.p.mats : nullptr; a.mout = mout ? c->ft.p.mats + RR : nullptr;
     if (kind < 2) {
         a.L = hg.Lx; a.ph = c->ft.p.ph1;
-        if (kind == 1) { a.threads = hg.thrx2; a.min_ = a.mout = nullptr; }
-        CK(c->ops->dir[kind == 0 ? VD_EXACT1 : VD_EXACT2](a, c->st));
+        if (kind == 1) CK(run_sub2(c, hg, d_in, d_out, c->ft.p.ph1));
+        else CK(c->ops->dir[VD_EXACT1](a, c->st));
     } else {
         a.threads = hg.thre; a.L = hg.Le; a.E = d_E; a.Q = c->ft.p.Q;
         a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1; a.f2a = c->ft.p.f2a; a.f2b = c->ft.p.f2b;

@@ -20,6 +20,7 @@ struct GridDev {
     const double* ksq1;      // [nh]  true k^2 by k1
     const double* ksq2p;     // [n]   true k^2 by stored position
     const double2* tw;       // [n/2] exp(-2 pi i k / n)
+    const double2* wtab;     // twiddle tables of the radix groups of wf_plan(log2n), see wfft.cuh (built by the host)
 };
 
 // Opt a kernel in to the whole dynamic shared memory of an SM of the CURRENT device.  cudaFuncSetAttribute is state
