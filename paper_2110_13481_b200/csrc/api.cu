@@ -84,6 +84,7 @@ struct dlr_ctx {
     double *partial, *partialP[3], *partialC, *partial2a;
     double *margp1, *margp2, *margV;         // marginals of V (k_marginals partial planes; M1, M2, M3 as 3 x [r][n_v])
     double *gram2, *pgram2[3], *colsum2;     // group sums of the per-CTA partial rows (group_prereduce)
+    double *gramF, *pgramF[3], *colsumF;     // and their totals (one row each): what the consumers read
     unsigned* grp_cnt;                       // 3 x DLR_CNT_STRIDE group counters, zero between kernels
     // small buffers
     double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *zsum, *mx, *mv, *mxp, *mvp, *mres, *esum;
@@ -255,6 +256,9 @@ size_t carve(dlr_ctx* c, char* base) {
     c->gram2 = cv.take<double>(groups * nvmax);
     for (int d = 0; d < 3; d++) c->pgram2[d] = cv.take<double>(groups * (size_t)(R * (R - 1) / 2));
     c->colsum2 = cv.take<double>(groups * (size_t)R);
+    c->gramF = cv.take<double>(nvmax);
+    for (int d = 0; d < 3; d++) c->pgramF[d] = cv.take<double>((size_t)(R * (R - 1) / 2));
+    c->colsumF = cv.take<double>(R);
     c->grp_cnt = cv.take<unsigned>(3 * DLR_CNT_STRIDE);
     {
         const size_t nv = (size_t)c->gv.g.n;
@@ -415,7 +419,7 @@ D1Args d1args(dlr_ctx* c, const HostGrid& hg) {
     D1Args a;
     memset(&a, 0, sizeof(a));
     a.g = hg.g; a.T = hg.T1; a.scale = 2.0 / (double)hg.g.N; a.threads = hg.thr1;
-    a.partial2 = c->gram2; a.grp_cnt = c->grp_cnt;
+    a.partial2 = c->gram2; a.partialF = c->gramF; a.grp_cnt = c->grp_cnt;
     return a;
 }
 
@@ -442,6 +446,7 @@ DirArgs dirargs(dlr_ctx* c, const HostGrid& hg) {
     memset(&a, 0, sizeof(a));
     a.g = hg.g; a.threads = hg.thrx;
     a.gram2 = c->gram2; a.colsum2 = c->colsum2; a.grp_cnt = c->grp_cnt;
+    a.gramF = c->gramF; a.colsumF = c->colsumF;
     return a;
 }
 int dir_blocks(const HostGrid& hg, int L) { return dir_tiles(hg.g.n, L); }
@@ -478,23 +483,24 @@ cudaError_t run_sub2(dlr_ctx* c, const HostGrid& hg, const double* in, double* o
 void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M1, double* colsum, double* T, double* lam) {
     const int R = c->R;
     DirArgs a = dirargs(c, hg);
-    a.in = A; a.E = c->E; a.L = hg.Lc; a.gram = c->partial; a.pgram = c->partialP[0]; a.pgram2 = c->pgram2[0]; a.threads = hg.thrc;
+    a.in = A; a.E = c->E; a.L = hg.Lc; a.gram = c->partial; a.pgram = c->partialP[0]; a.pgram2 = c->pgram2[0]; a.pgramF = c->pgramF[0];
+    a.threads = hg.thrc;
     CK(c->ops->dir[kind == 1 ? VD_COEFF1_V : VD_COEFF1_E](a, c->st));
     c->bytes_acc += 3.0 * fac_bytes(c, hg) + (kind == 2 ? 24.0 * (double)hg.g.N : 0.0);
     // fork: M1 and its eigen-decomposition need only the Gram sums of the pass above; they run beside the two
     // remaining passes (under stream capture this becomes a parallel branch of the step graph)
     CK(cudaEventRecord(c->ev_fork, c->st));
     CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->gram2, dlr_groups(dir_blocks(hg, hg.Lc)), R, kind == 1, hg.g.h3, M1, colsum, T, lam,
+    k_coeff1_eig<<<3, DLR_EIG_THREADS, 0, c->side>>>(c->gramF, 1, R, kind == 1, hg.g.h3, M1, colsum, T, lam,
                                                      (kind == 1 ? c->tc_warm : c->td_warm) ? 1 : 0, c->status);
     CK(cudaGetLastError());
     (kind == 1 ? c->tc_warm : c->td_warm) = true;
     CK(cudaEventRecord(c->ev_join, c->side));
     c->count_launches -= 3;                         // the three event calls above are not kernel launches
     a.gram = nullptr; a.E = nullptr;
-    a.pgram = c->partialP[1]; a.pgram2 = c->pgram2[1];
+    a.pgram = c->partialP[1]; a.pgram2 = c->pgram2[1]; a.pgramF = c->pgramF[1];
     CK(c->ops->dir[VD_COEFF2](a, c->st));
-    a.pgram = c->partialP[2]; a.pgram2 = c->pgram2[2];
+    a.pgram = c->partialP[2]; a.pgram2 = c->pgram2[2]; a.pgramF = c->pgramF[2];
     CK(c->ops->dir[VD_COEFF3](a, c->st));
     CK(cudaStreamWaitEvent(c->st, c->ev_join, 0));  // join before anything reads M1, T, lam, colsum
     c->count_launches -= 1;
@@ -538,8 +544,8 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
     memset(&a, 0, sizeof(a));
     a.R = c->R;
     if (m2) {
-        a.do_m2 = 1; a.nblocks = dlr_groups(dir_blocks(*m2->hg, m2->hg->Lc));
-        for (int d = 0; d < 3; d++) a.pgram[d] = c->pgram2[d];
+        a.do_m2 = 1;
+        for (int d = 0; d < 3; d++) a.pgram[d] = c->pgramF[d];             // the totals of the three coefficient passes
         a.m2scale = m2->hg->g.h3 / (double)m2->hg->g.n; a.M2 = m2->M2;     // 1D Parseval: sum_x u dv = (1/n) sum_k ...
     }
     if (sf) { a.do_s = 1; a.S = sf->S; a.ts = sf->t; a.C1 = c->C1; a.C2 = c->C2; a.D1 = c->D1; a.D2 = c->D2; }
@@ -547,9 +553,7 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
         a.do_tab = 1; a.Tm = tb->T; a.lam = tb->lam; a.Sin = tb->Sin; a.transS = tb->transS; a.g = tb->hg->g;
         a.sgn = tb->sgn; a.tsub = tb->tsub; a.t3 = tb->t3; a.M2c = tb->M2c; a.nlsign = tb->nlsign; a.o = c->ft.p;
     }
-    const size_t sm = sf ? (size_t)12 * c->R * c->R * sizeof(double) : 0;     // staged C1, C2, D1, D2
-    k_post<<<1, DLR_SMALL_THREADS, sm, c->st>>>(a);
-    CK(cudaGetLastError());
+    CK(c->ops->post(a, c->st));
 }
 
 // Electric field from rho = A * p (p holds the minus sign and the quadrature weight): eqs. (12)/(13) + Poisson
@@ -594,22 +598,21 @@ void field_join(dlr_ctx* c) {
 
 // shifted CholeskyQR3 of KL (N x r) -> orthonormal basis (h^3 B^T B = I) into `basis`, coupling matrix into Sout
 // (transS: S = R^T for the L step, Fig. 1 line 40 transpose_inplace).
-// The Gram sums of KL must already be in c->partial, one row per CTA of the pass that produced KL (nblocks0 rows).
-void qr(dlr_ctx* c, const HostGrid& hg, int nblocks0, double* basis, double* Sout, int transS) {
+// The total of the Gram sums of KL must already be in c->gramF (written by the last pass of the flow).  Three A*Mat
+// passes; the r x r factorisation of each stage happens in the prologue of its own pass (chol_warp.cuh).  Stage 1
+// decides on the device whether the third is needed (only while kappa(K) >~ 1e7, i.e. the first few steps): if not it
+// writes the basis itself and the stage-2 launch returns at once.
+void qr(dlr_ctx* c, const HostGrid& hg, double* basis, double* Sout, int transS) {
     const int R = c->R;
-    const double shift = 64.0 * R * 2.220446049250313e-16;
-    const double osc = 1.0 / sqrt(hg.g.h3), ssc = sqrt(hg.g.h3);
     double* src[3] = {c->KL, c->Q1, c->KL};
     double* dst[3] = {c->Q1, c->KL, basis};
     for (int stage = 0; stage < 3; stage++) {
-        // stage 0 reads the Gram sums written by the last pass of the flow (nblocks0 tiles), later stages those of
-        // the previous A*Mat pass
-        k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->gram2, dlr_groups(stage == 0 ? nblocks0 : d1_blocks(hg)), R, stage, stage == 2, shift, osc, ssc,
-                                                          transS, c->apply, c->Rtot, Sout, c->status, c->status + 1);
-        CK(cudaGetLastError());
         D1Args a = d1args(c, hg);
-        a.in_real = src[stage]; a.out_real = dst[stage]; a.mat = c->apply; a.partial = c->partial;
-        if (stage >= 1) { a.skip_flag = c->status + 1; a.skip_mode = stage; a.out_alt = basis; }
+        a.in_real = src[stage]; a.out_real = dst[stage]; a.out_alt = basis; a.partial = c->partial;
+        a.ch.gsum = c->gramF; a.ch.stage = stage; a.ch.transS = transS;
+        a.ch.shift = 64.0 * R * 2.220446049250313e-16;
+        a.ch.out_scale = 1.0 / sqrt(hg.g.h3); a.ch.s_scale = sqrt(hg.g.h3);
+        a.ch.Rtot = c->Rtot; a.ch.Sout = Sout; a.ch.status = c->status; a.ch.qrflag = c->status + 1;
         if (stage < 2) c->bytes_acc += 2.0 * fac_bytes(c, hg);     // the third stage is skipped in steady state: not counted
         CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
     }
@@ -618,9 +621,8 @@ void qr(dlr_ctx* c, const HostGrid& hg, int nblocks0, double* basis, double* Sou
 // K- or L-flow of section 4 of the factor `src` (X or V; the product with the coupling matrix is
 // folded into the first column-mixing matrix).  order 1: Lie + exponential Euler = 3 directional passes;
 // order 2: Strang + ETD2RK = 5 passes (1, 2, 3, 2, 1).  Result: real factor in c->KL with its Gram sums in c->partial,
-// or (zero_only) only the column sums of the result (without the h^3 weight) in c->zsum.  Returns the number of
-// Gram partial rows written.
-int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order, bool zero_only) {
+// or (zero_only) only the column sums of the result (without the h^3 weight) in c->zsum.
+void flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order, bool zero_only) {
     const RankOps* ops = c->ops;
     const int RR = c->R * c->R;
     const double* mats = c->ft.p.mats;
@@ -644,17 +646,16 @@ int flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int order
         else { e.store = 1; e.out = c->KL; e.gram = c->partial; }
         CK(ops->dir[is_L ? VD_ETD1_V : VD_ETD1_E](e, c->st));
         if (zero_only) {
-            k_colsum_reduce<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->colsum2, dlr_groups(dir_blocks(hg, hg.Le)), c->R, c->zsum);
+            k_colsum_reduce<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->colsumF, 1, c->R, c->zsum);
             CK(cudaGetLastError());
         }
-        return dir_blocks(hg, hg.Le);
+        return;
     }
     e.mout = mats + 5 * RR; e.store = 1; e.out = c->W;          // T3^T T2
     CK(ops->dir[is_L ? VD_ETD2_V : VD_ETD2_E](e, c->st));
     CK(run_sub2(c, hg, c->W, c->W, c->ft.p.ph2));                // sub-flow 2, second half
     a.out = c->KL; a.min_ = mats + 6 * RR; a.mout = mats + 7 * RR; a.ph = c->ft.p.ph1; a.gram = c->partial;
     CK(ops->dir[VD_EXACT1](a, c->st));                           // sub-flow 1, second half, + Gram of the result
-    return dir_blocks(hg, hg.Lx);
 }
 
 // one step, issued on c->st (directly or under stream capture)
@@ -684,9 +685,9 @@ void issue_step(dlr_ctx* c, double tau) {
         const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, tp, tp, c->C2, 1.0};
         post(c, nullptr, nullptr, &tb);
     }
-    int nb = flow(c, gx, c->X, false, 1, false);
+    flow(c, gx, c->X, false, 1, false);
     phase_mark(c, "K step (predictor)");
-    qr(c, gx, nb, Xp, Sp, 0);
+    qr(c, gx, Xp, Sp, 0);
     phase_mark(c, "QR K (predictor)");
     // ---- line 6: D coefficients from X1 and E0;  line 7: S step;  lines 8-9: L0 = V0 S2^T, tables of the L step
     coeffs(c, gx, Xp, 2, c->D1, nullptr, c->TD, c->lamD);
@@ -698,9 +699,9 @@ void issue_step(dlr_ctx* c, double tau) {
     }
     phase_mark(c, "S step (predictor)");
     if (order == 1) {
-        nb = flow(c, gv, c->V, true, 1, false);
+        flow(c, gv, c->V, true, 1, false);
         phase_mark(c, "L step");
-        qr(c, gv, nb, c->V, c->S, 1);                 // line 10: V1, S3 = R^T
+        qr(c, gv, c->V, c->S, 1);                 // line 10: V1, S3 = R^T
         phase_mark(c, "QR L");
         c->vh_valid = false;
         c->bytes_step = c->bytes_acc;
@@ -719,9 +720,9 @@ void issue_step(dlr_ctx* c, double tau) {
         const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0};
         post(c, nullptr, nullptr, &tb);
     }
-    nb = flow(c, gx, c->X, false, 2, false);
+    flow(c, gx, c->X, false, 2, false);
     phase_mark(c, "first K step");
-    qr(c, gx, nb, c->X, c->S, 0);
+    qr(c, gx, c->X, c->S, 0);
     phase_mark(c, "QR K (first)");
     // ---- line 5: D coefficients from X2 and E^{1/2};  line 6: S step;  tables of the L step (L = V0 S4^T)
     coeffs(c, gx, c->X, 2, c->D1, nullptr, c->TD, c->lamD);
@@ -733,9 +734,9 @@ void issue_step(dlr_ctx* c, double tau) {
     }
     phase_mark(c, "first S step");
     // ---- lines 7-9: L step (Strang) of length tau, QR -> V1, S5 = R^T
-    nb = flow(c, gv, c->V, true, 2, false);
+    flow(c, gv, c->V, true, 2, false);
     phase_mark(c, "L step");
-    qr(c, gv, nb, c->V, c->S, 1);
+    qr(c, gv, c->V, c->S, 1);
     phase_mark(c, "QR L");
     // ---- line 10: C coefficients from V1 (they are also the next step's line-1 coefficients);  line 11: S step;
     //      tables of the second K step (K3 = X2 S6)
@@ -749,9 +750,9 @@ void issue_step(dlr_ctx* c, double tau) {
     }
     phase_mark(c, "second S step");
     // ---- lines 12-14: K step (Strang) of length tau/2, QR -> X3, S7
-    nb = flow(c, gx, c->X, false, 2, false);
+    flow(c, gx, c->X, false, 2, false);
     phase_mark(c, "second K step");
-    qr(c, gx, nb, c->X, c->S, 0);
+    qr(c, gx, c->X, c->S, 0);
     phase_mark(c, "QR K (second)");
     c->vh_valid = true;
     c->bytes_step = c->bytes_acc;
@@ -809,7 +810,6 @@ static cudaError_t configure_kernels(dlr_ctx* c) {
     OPTIN(k_d3<3, 3, D3_INV_ONLY, false>);
     OPTIN(k_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>);
     OPTIN(k_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>);
-    OPTIN(k_post);
     if (e == cudaSuccess) e = configure_sub2();
     OPTIN(k_lpred_sums);
 #undef OPTIN
@@ -1119,10 +1119,11 @@ int dlr_test_chol_decide(dlr_ctx* c, const double* gram_upper, int* third_stage_
     cudaError_t e = cudaMemcpyAsync(c->gram2, gram_upper, P * sizeof(double), cudaMemcpyHostToDevice, c->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(st_before, c->status, sizeof(st_before), cudaMemcpyDeviceToHost, c->st);
     if (e != cudaSuccess) return fail(c, e, "dlr_test_chol_decide");
-    // stage 1 of the CholeskyQR of a factor whose once-orthogonalised Gram matrix is gram_upper (one partial row)
-    k_chol_stage<<<1, DLR_SMALL_THREADS, 0, c->st>>>(c->gram2, 1, R, 1, 0, 0.0, 1.0, 1.0, 0, c->apply, c->Rtot, c->Sp,
-                                                      c->status, c->status + 1);
-    CK(cudaGetLastError());
+    // stage 1 of the CholeskyQR of a factor whose once-orthogonalised Gram matrix is gram_upper (the total row)
+    CholArgs ca;
+    ca.gsum = c->gram2; ca.stage = 1; ca.transS = 0; ca.shift = 0.0; ca.out_scale = 1.0; ca.s_scale = 1.0;
+    ca.Rtot = c->Rtot; ca.Sout = c->Sp; ca.status = c->status; ca.qrflag = c->status + 1;
+    CK(c->ops->chol_test(ca, c->apply, c->st));
     e = cudaMemcpyAsync(st_after, c->status, sizeof(st_after), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->status, st_before, sizeof(st_before), cudaMemcpyHostToDevice, c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);

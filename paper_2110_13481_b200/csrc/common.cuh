@@ -158,15 +158,18 @@ __device__ __forceinline__ void fft_lines(double2* s, int LP, int nlines, int lo
     }
 }
 
-// ---------------------------------------------------------------- two-level deterministic partial sums
+// ---------------------------------------------------------------- three-level deterministic partial sums
 // A producer CTA writes its partial row rows[blockIdx.x][0..nvals); the LAST CTA to finish of every group of DLR_GRP
-// consecutive CTAs then adds the group's rows in index order into rows2[group][0..nvals).  The result does not depend
-// on which CTA does it, so the sums stay bit-reproducible; the single-CTA consumer only reads gridDim.x / DLR_GRP
-// rows.  counters[group] must be 0 on entry and is 0 again on exit (atomicInc wraps).
+// consecutive CTAs then adds the group's rows in index order into rows2[group][0..nvals), and the last GROUP to finish
+// adds the group sums in index order into final_row[0..nvals) (if not nullptr).  The result does not depend on which
+// CTA does it, so the sums stay bit-reproducible; a consumer reads one row.  counters[group] and the grid-level counter
+// counters[DLR_CNT_STRIDE - 1] must be 0 on entry and are 0 again on exit (atomicInc wraps).
 #define DLR_GRP 16
+#define DLR_CNT_STRIDE 4096
 __host__ __device__ inline int dlr_groups(int nblocks) { return (nblocks + DLR_GRP - 1) / DLR_GRP; }
 
-__device__ __forceinline__ void group_prereduce(const double* rows, int nvals, unsigned* counters, double* rows2) {
+__device__ __forceinline__ void group_prereduce(const double* rows, int nvals, unsigned* counters, double* rows2,
+                                                double* final_row = nullptr) {
     __shared__ int s_last;
     __threadfence();
     __syncthreads();
@@ -181,6 +184,21 @@ __device__ __forceinline__ void group_prereduce(const double* rows, int nvals, u
         double s = 0.0;
         for (int b = 0; b < cnt; b++) s += __ldcg(p + (size_t)b * nvals);     // L2 (other CTAs wrote these)
         rows2[(size_t)grp * nvals + v] = s;
+    }
+    if (final_row == nullptr) return;
+    const int ngrp = dlr_groups((int)gridDim.x);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0)
+        s_last = (atomicInc(counters + DLR_CNT_STRIDE - 1, (unsigned)(ngrp - 1)) == (unsigned)(ngrp - 1));
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int v = threadIdx.x; v < nvals; v += blockDim.x) {
+        const double* p = rows2 + v;
+        double s = 0.0;
+        for (int g = 0; g < ngrp; g++) s += __ldcg(p + (size_t)g * nvals);
+        final_row[v] = s;
     }
 }
 

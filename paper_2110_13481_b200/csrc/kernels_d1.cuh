@@ -9,6 +9,7 @@
 #pragma once
 #include "common.cuh"
 #include "gram_mma.cuh"
+#include "chol_warp.cuh"
 
 enum { D1_IN_REAL = 0, D1_IN_CPLX = 1 };
 enum { D1_OP_NONE = 0, D1_OP_MATVEC = 1 };
@@ -24,9 +25,11 @@ struct D1Args {
     const double* mat;         // MATVEC: [RIN][ROUT]
     double* partial;           // [gridDim.x][nvals] Gram partial sums
     double* partial2;          // [groups][nvals] group sums (see group_prereduce), or nullptr
+    double* partialF;          // [nvals] their sum (the row a consumer reads), or nullptr
     unsigned* grp_cnt;         // group counters
-    const int* skip_flag;      // adaptive CholeskyQR (see k_chol_stage): if *skip_flag != 0 then
-    int skip_mode;             //   mode 1: write out_alt instead of out_real;  mode 2: the whole launch is a no-op
+    CholArgs ch;               // MATVEC with ch.gsum != nullptr: the matrix is the CholeskyQR stage of chol_warp.cuh, done by
+                               //   warp 0 of every CTA.  Stage 1 that turns out to be the last one writes out_alt (the
+                               //   basis) without a Gram; a stage-2 launch returns at once when ch.qrflag[0] != 0
     double* out_alt;
     double scale;              // applied to the data after a complex input (2/N for an inverse transform)
     int T;                     // rows per CTA (power of two dividing n^2)
@@ -74,13 +77,23 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 16 
     const int tid = threadIdx.x, nth = blockDim.x;
     double* out_real = a.out_real;
     bool want_gram = true;
-    if (a.skip_flag != nullptr && *a.skip_flag != 0) {
-        if (a.skip_mode == 2) return;
-        if (a.skip_mode == 1) { out_real = a.out_alt; want_gram = false; }     // this pass is the last one: no Gram
+    constexpr bool CHOL = (OP == D1_OP_MATVEC && RIN == ROUT && RIN > 3);
+    __shared__ int s_chol_last;
+    bool chol = false;
+    if constexpr (CHOL) {
+        chol = a.ch.gsum != nullptr;
+        if (chol && a.ch.stage == 2 && a.ch.qrflag[0] != 0) return;       // third stage not needed
     }
 
     for (int i = tid; i < M; i += nth) tw[i] = a.g.tw[i];
-    if (OP == D1_OP_MATVEC && ROUT == 1 && a.rho_vec != nullptr) {
+    if (chol) {
+        if constexpr (CHOL) {
+            if (tid < 32) {
+                const bool last = chol_warp<RIN>(a.ch, mat, blockIdx.x == 0);
+                if (tid == 0) s_chol_last = last ? 1 : 0;
+            }
+        }
+    } else if (OP == D1_OP_MATVEC && ROUT == 1 && a.rho_vec != nullptr) {
         for (int i = tid; i < RIN; i += nth) {
             double sacc = 0.0;
             if (a.rho_S != nullptr)
@@ -97,14 +110,19 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 16 
     // ------------------------------------------------------------------ load
     if (IN_MODE == D1_IN_REAL) {
         const int cnt = T * M;
-        for (int c = 0; c < RIN; c++) {
-            const double2* src = (const double2*)(a.in_real + (size_t)c * a.g.N) + q0 * M;
-            for (int i = tid; i < cnt; i += nth) {
-                const int t = i >> logM, j = i & (M - 1);
-                z[(size_t)j * LP + c * T + t] = src[i];
+        // warp 0 is busy with the factorisation: the other warps load the tile meanwhile
+        const int ltid = chol ? tid - 32 : tid, lnth = chol ? nth - 32 : nth;
+        if (ltid >= 0) {
+            for (int c = 0; c < RIN; c++) {
+                const double2* src = (const double2*)(a.in_real + (size_t)c * a.g.N) + q0 * M;
+                for (int i = ltid; i < cnt; i += lnth) {
+                    const int t = i >> logM, j = i & (M - 1);
+                    z[(size_t)j * LP + c * T + t] = src[i];
+                }
             }
         }
         __syncthreads();
+        if (chol && a.ch.stage == 1 && s_chol_last) { out_real = a.out_alt; want_gram = false; }   // last stage: no Gram
     } else {
         // half-spectrum row Ah[0..M] -> Z[k] = Ze[k] + i Zo[k] at bit-reversed positions, then inverse FFT
         const int nk = (M >> 1) + 1, nh = a.g.nh;
@@ -213,7 +231,7 @@ __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 16 
         });
     }
     if (GRAM != D1_GRAM_NONE && want_gram && a.partial2 != nullptr)
-        group_prereduce(a.partial, d1_gram_nvals(ROUT, GRAM), a.grp_cnt, a.partial2);
+        group_prereduce(a.partial, d1_gram_nvals(ROUT, GRAM), a.grp_cnt, a.partial2, a.partialF);
 }
 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>

@@ -24,7 +24,6 @@
 
 enum { DOP_EXACT = 0, DOP_ETD1 = 1, DOP_ETD2 = 2, DOP_COEFF = 3 };
 enum { DW_NONE = 0, DW_E = 1, DW_V = 2 };
-#define DLR_CNT_STRIDE 4096
 
 struct DirArgs {
     GridDev g;
@@ -40,6 +39,7 @@ struct DirArgs {
     double* pgram;         // COEFF: per-CTA Parseval partial sums [grid][R(R-1)/2]
     double* colsum;        // per-CTA column sums of the output [grid][R], or nullptr
     double *gram2, *pgram2, *colsum2;   // group sums of the three (see group_prereduce)
+    double *gramF, *pgramF, *colsumF;   // and their totals: the single row a consumer reads
     unsigned* grp_cnt;     // group counters: [0..) gram, [DLR_CNT_STRIDE..) pgram, [2 DLR_CNT_STRIDE..) colsum
     int L;                 // packed lines per column in a tile (power of two)
     int store;             // write `out`
@@ -318,9 +318,9 @@ k_dir(const DirArgs a) {
         }
         if (WG && a.gram != nullptr) {
             constexpr int NV = 3 * P + (DW == DW_V ? R : 0);
-            group_prereduce(a.gram, NV, a.grp_cnt, a.gram2);
+            group_prereduce(a.gram, NV, a.grp_cnt, a.gram2, a.gramF);
         }
-        group_prereduce(a.pgram, P2, a.grp_cnt + DLR_CNT_STRIDE, a.pgram2);
+        group_prereduce(a.pgram, P2, a.grp_cnt + DLR_CNT_STRIDE, a.pgram2, a.pgramF);
         return;
     }
 
@@ -485,9 +485,9 @@ k_dir(const DirArgs a) {
             const int ca = 8 * I + i, cb = 8 * J + j;
             if (ca <= cb && cb < R) part[upper_pair_index(R, ca, cb)] = v;
         });
-        group_prereduce(a.gram, P, a.grp_cnt, a.gram2);
+        group_prereduce(a.gram, P, a.grp_cnt, a.gram2, a.gramF);
     }
-    if (a.colsum != nullptr) group_prereduce(a.colsum, R, a.grp_cnt + 2 * DLR_CNT_STRIDE, a.colsum2);
+    if (a.colsum != nullptr) group_prereduce(a.colsum, R, a.grp_cnt + 2 * DLR_CNT_STRIDE, a.colsum2, a.colsumF);
 }
 
 template <int R, int DIR, int DOP, int DW>

@@ -10,6 +10,11 @@
 namespace {
 constexpr int R = DLR_RANK;
 
+cudaError_t launch_chol_test(const CholArgs& ca, double* mat_out, cudaStream_t st) {
+    k_chol_test<R><<<1, 32, 0, st>>>(ca, mat_out);
+    return cudaGetLastError();
+}
+
 cudaError_t configure_rank() {
     cudaError_t e = cudaSuccess;
 #define OPTIN(...) if (e == cudaSuccess) e = dlr_optin_smem(__VA_ARGS__)
@@ -27,6 +32,7 @@ cudaError_t configure_rank() {
     OPTIN(k_dir<R, 1, DOP_COEFF, DW_E>);
     OPTIN(k_dir<R, 2, DOP_COEFF, DW_NONE>);
     OPTIN(k_dir<R, 3, DOP_COEFF, DW_NONE>);
+    OPTIN(k_post<R>);
 #undef OPTIN
     return e;
 }
@@ -53,6 +59,8 @@ extern "C" const RankOps* CAT(dlr_rank_ops_, DLR_RANK)() {
             launch_dir<R, 1, DOP_COEFF, DW_E>,
             launch_dir<R, 2, DOP_COEFF, DW_NONE>,
             launch_dir<R, 3, DOP_COEFF, DW_NONE>,
-        }};
+        },
+        launch_post<R>,
+        launch_chol_test};
     return &ops;
 }

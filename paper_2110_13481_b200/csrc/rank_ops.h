@@ -5,6 +5,7 @@
 #include "kernels_d2.cuh"
 #include "kernels_d3.cuh"
 #include "kernels_dir.cuh"
+#include "post.cuh"
 
 // row-tile kernels without a transform (CholeskyQR passes, density, initial-state check)
 enum {
@@ -34,6 +35,8 @@ struct RankOps {
     cudaError_t (*configure)();      // shared-memory opt-in of every kernel below on the current device (dlr_create)
     cudaError_t (*d1[V1_COUNT])(const D1Args&, cudaStream_t);
     cudaError_t (*dir[VD_COUNT])(const DirArgs&, cudaStream_t);
+    cudaError_t (*post)(const PostArgs&, cudaStream_t);           // r x r work between two streaming phases (post.cuh)
+    cudaError_t (*chol_test)(const CholArgs&, double* mat_out, cudaStream_t);     // one CholeskyQR stage on its own (test hook)
 };
 
 const RankOps* dlr_rank_ops(int R);      // nullptr if the rank is not compiled in

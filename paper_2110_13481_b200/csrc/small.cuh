@@ -5,6 +5,7 @@
 // (the C ABI layout).
 #pragma once
 #include "common.cuh"
+#include "flowtab.cuh"
 
 #define DLR_G1 32          // number of second-level partial rows
 #define DLR_RMAXS 24       // largest rank the small kernels are dimensioned for
@@ -211,333 +212,11 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// phi functions of a purely imaginary argument z = i*theta (reading R7): closed forms for |theta| >= 1,
-// Taylor series below.
-__device__ const double DLR_INV_FACT[24] = {      // 1/k!, k = 1..24 (correctly rounded)
-    1.0, 0.5, 0.16666666666666666, 0.041666666666666664,
-    0.008333333333333333, 0.001388888888888889, 0.0001984126984126984, 2.48015873015873e-05,
-    2.7557319223985893e-06, 2.755731922398589e-07, 2.505210838544172e-08, 2.08767569878681e-09,
-    1.6059043836821613e-10, 1.1470745597729725e-11, 7.647163731819816e-13, 4.779477332387385e-14,
-    2.8114572543455206e-15, 1.5619206968586225e-16, 8.22063524662433e-18, 4.110317623312165e-19,
-    1.9572941063391263e-20, 8.896791392450574e-22, 3.868170170630684e-23, 1.6117375710961184e-24};
-__device__ inline void phi12_imag(double th, double2& p1, double2& p2) {
-    if (fabs(th) < 1.0) {
-        // Horner in z = i th:  phi1 = sum z^m/(m+1)!,  phi2 = sum z^m/(m+2)!
-        double2 s1 = make_double2(0.0, 0.0), s2 = s1;
-        for (int m = 21; m >= 0; m--) {
-            // s = s*z + coeff,  z = (0, th)
-            s1 = make_double2(-s1.y * th + DLR_INV_FACT[m], s1.x * th);
-            s2 = make_double2(-s2.y * th + DLR_INV_FACT[m + 1], s2.x * th);
-        }
-        p1 = s1; p2 = s2;
-    } else {
-        double sn, cs, sh, ch;
-        sincos(th, &sn, &cs);
-        sincos(0.5 * th, &sh, &ch);
-        const double omc = 2.0 * sh * sh;      // 1 - cos(th)
-        (void)cs; (void)ch;
-        p1 = make_double2(sn / th, omc / th);
-        p2 = make_double2(omc / (th * th), (th - sn) / (th * th));
-    }
-}
-
-// Tables of one K- or L-flow (see D3Args).  Tm: 3 x [R][R] eigenvectors (columns), lam: 3 x [R];
-// Sin: r x r column-major coupling matrix; transS = 0: A0 = Sin*T1 (K = X S), 1: A0 = Sin^T*T1 (L = V S^T).
-// sgn = -1 (K equation (9)) or +1 (L equation (11)); tsub = length of sub-flows 1,2; t3 = length of sub-flow 3.
-// M2c: 3 x [R][R] derivative coefficients; nl gets nlsign * M2c (matrices of the real-space term).
-struct FlowTabPtrs {
-    double* mats;   // 8 R^2: 0 Sin*T1, 1 T1^T T2, 2 T2^T T3, 3 T3^T, 4 T3, 5 T3^T T2, 6 T2^T T1, 7 T1^T  ([cin][cout])
-    double* Q;      // 3 R^2: real-space term in the eigenbasis of direction 3, Q_i = T3^T nl_i^T T3, nl_i = nlsign * M2c_i
-    double2 *ph1, *ph2, *ez, *f1, *f2a, *f2b;   // [n][R] each, by stored (bit-reversed) position
-};
-
-__device__ __forceinline__ void dev_flow_tables(const double* Tm, const double* lam, const double* Sin, int transS,
-                                                int R, const GridDev& g, double sgn, double tsub, double t3,
-                                                const double* M2c, double nlsign, const FlowTabPtrs& o,
-                                                double* scratch /* shared, >= 7 R^2 doubles */) {
-    const double* T1 = Tm;
-    const double* T2 = Tm + R * R;
-    const double* T3 = Tm + 2 * R * R;
-    const int RR = R * R;
-    for (int idx = threadIdx.x; idx < RR; idx += blockDim.x) {
-        const int a = idx / R, b = idx % R;
-        double m0 = 0, m1 = 0, m2 = 0, m5 = 0, m6 = 0;
-        for (int k = 0; k < R; k++) {
-            const double s_ak = transS ? Sin[k + R * a] : Sin[a + R * k];
-            m0 = fma(s_ak, T1[k * R + b], m0);
-            m1 = fma(T1[k * R + a], T2[k * R + b], m1);
-            m2 = fma(T2[k * R + a], T3[k * R + b], m2);
-            m5 = fma(T3[k * R + a], T2[k * R + b], m5);
-            m6 = fma(T2[k * R + a], T1[k * R + b], m6);
-        }
-        o.mats[0 * RR + idx] = m0;
-        o.mats[1 * RR + idx] = m1;
-        o.mats[2 * RR + idx] = m2;
-        o.mats[3 * RR + idx] = T3[b * R + a];
-        o.mats[4 * RR + idx] = T3[idx];
-        o.mats[5 * RR + idx] = m5;
-        o.mats[6 * RR + idx] = m6;
-        o.mats[7 * RR + idx] = T1[b * R + a];
-    }
-    // N(A) T3 = sum_i diag(w_i) (A T3) (T3^T nl_i^T T3):  Q_i = T3^T (nl_i^T T3), two r^3 products through shared memory
-    {
-        double* T3s = scratch;                 // [R][R]
-        double* nls = scratch + RR;            // 3 x [R][R]
-        double* tmpm = scratch + 4 * RR;       // 3 x [R][R]: nl_i^T T3
-        for (int idx = threadIdx.x; idx < RR; idx += blockDim.x) T3s[idx] = T3[idx];
-        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) nls[idx] = M2c[idx];
-        __syncthreads();
-        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) {
-            const int d = idx / RR, e = idx - d * RR, pp = e / R, b = e - pp * R;
-            double t = 0.0;
-            for (int qq = 0; qq < R; qq++) t = fma(nls[d * RR + qq * R + pp], T3s[qq * R + b], t);
-            tmpm[idx] = t;
-        }
-        __syncthreads();
-        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) {
-            const int d = idx / RR, e = idx - d * RR, a = e / R, b = e - a * R;
-            double q = 0.0;
-            for (int pp = 0; pp < R; pp++) q = fma(T3s[pp * R + a], tmpm[d * RR + pp * R + b], q);
-            o.Q[idx] = nlsign * q;
-        }
-    }
-    const int n = g.n;
-    for (int idx = threadIdx.x; idx < n * R; idx += blockDim.x) {
-        const int k = idx / R, j = idx % R;
-        double sn, cs;
-        sincos(sgn * tsub * g.kt2p[k] * lam[j], &sn, &cs);
-        o.ph1[idx] = make_double2(cs, sn);
-        sincos(sgn * tsub * g.kt2p[k] * lam[R + j], &sn, &cs);
-        o.ph2[idx] = make_double2(cs, sn);
-        const double th = sgn * t3 * g.kt2p[k] * lam[2 * R + j];
-        sincos(th, &sn, &cs);
-        o.ez[idx] = make_double2(cs, sn);
-        double2 p1, p2;
-        phi12_imag(th, p1, p2);
-        o.f1[idx] = make_double2(t3 * p1.x, t3 * p1.y);
-        o.f2a[idx] = make_double2(t3 * (p1.x - p2.x), t3 * (p1.y - p2.y));
-        o.f2b[idx] = make_double2(t3 * p2.x, t3 * p2.y);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// S step: one classical RK4 step of eq. (10):  dS/dt = sum_i D2_i S C1_i^T - D1_i S C2_i^T
-#define DLR_RR 400          // r^2 for the largest supported rank (20)
-struct SflowScratch {
-    double Sc[DLR_RR], Y[DLR_RR], Kacc[DLR_RR], Pm[3][DLR_RR], Qm[3][DLR_RR];
-};
-__device__ __forceinline__ void dev_sflow(double* S, int R, double t, const double* C1, const double* C2,
-                                          const double* D1, const double* D2, SflowScratch& sc) {
-    double (&Sc)[DLR_RR] = sc.Sc;
-    double (&Y)[DLR_RR] = sc.Y;
-    double (&Kacc)[DLR_RR] = sc.Kacc;
-    double (&Pm)[3][DLR_RR] = sc.Pm;
-    double (&Qm)[3][DLR_RR] = sc.Qm;
-    const int RR = R * R;
-    for (int i = threadIdx.x; i < RR; i += blockDim.x) { Sc[i] = S[i]; Y[i] = S[i]; Kacc[i] = 0.0; }
-    __syncthreads();
-    const double cw[4] = {1.0, 2.0, 2.0, 1.0}, cs[4] = {0.5, 0.5, 1.0, 0.0};
-    for (int stage = 0; stage < 4; stage++) {
-        // P_d = Y C1_d^T, Q_d = Y C2_d^T     (Y column-major: Y(a,k) = Y[a + R k])
-        for (int idx = threadIdx.x; idx < 3 * RR; idx += blockDim.x) {
-            const int d = idx / RR, a = (idx % RR) / R, b = idx % R;
-            double p = 0, q = 0;
-            for (int k = 0; k < R; k++) {
-                const double y = Y[a + R * k];
-                p = fma(y, C1[d * RR + b * R + k], p);
-                q = fma(y, C2[d * RR + b * R + k], q);
-            }
-            Pm[d][a * R + b] = p;
-            Qm[d][a * R + b] = q;
-        }
-        __syncthreads();
-        double rhs_reg[4];      // each thread owns entries idx = tid + m*blockDim (R^2 <= 4*256)
-        int m = 0;
-        for (int idx = threadIdx.x; idx < RR; idx += blockDim.x, m++) {
-            const int a = idx % R, b = idx / R;       // column-major entry (a,b)
-            double r = 0;
-            for (int d = 0; d < 3; d++)
-                for (int k = 0; k < R; k++)
-                    r += D2[d * RR + a * R + k] * Pm[d][k * R + b] - D1[d * RR + a * R + k] * Qm[d][k * R + b];
-            rhs_reg[m] = r;
-        }
-        __syncthreads();
-        m = 0;
-        for (int idx = threadIdx.x; idx < RR; idx += blockDim.x, m++) {
-            Kacc[idx] += cw[stage] * rhs_reg[m];
-            Y[idx] = Sc[idx] + cs[stage] * t * rhs_reg[m];
-        }
-        __syncthreads();
-    }
-    for (int i = threadIdx.x; i < RR; i += blockDim.x) S[i] = Sc[i] + (t / 6.0) * Kacc[i];
-    __syncthreads();
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// The r x r work between two streaming phases in ONE launch (single CTA), each part optional:
-//   do_m2 : derivative coefficients M2_i = h^3 A^T d_i A (antisymmetric) from the 1D Parseval
-//           partial sums of the three coefficient passes: pgram[d] [nblocks][P2], entry (a<b) at pe2;
-//   do_s  : S step, one RK4 step of eq. (10);
-//   do_tab: tables of the next K- or L-flow (mode-mixing matrices, phases, phi functions).
-struct PostArgs {
-    int R, do_m2, do_s, do_tab;
-    const double* pgram[3]; int nblocks; double m2scale; double* M2;
-    double* S; double ts; const double *C1, *C2, *D1, *D2;
-    const double *Tm, *lam, *Sin; int transS; GridDev g; double sgn, tsub, t3; const double* M2c; double nlsign;
-    FlowTabPtrs o;
-};
-
-__global__ void __launch_bounds__(DLR_SMALL_THREADS) k_post(const PostArgs a) {
-    __shared__ SflowScratch sc;
-    __shared__ double red[DLR_RMAXS * (DLR_RMAXS - 1) / 2], tmp[DLR_SMALL_THREADS];
-    const int R = a.R, RR = R * R;
-    if (a.do_m2) {
-        const int P2 = R * (R - 1) / 2;
-        for (int d = 0; d < 3; d++) {
-            cta_reduce_rows(a.pgram[d], a.nblocks, P2, 0, P2, red, tmp);
-            for (int idx = threadIdx.x; idx < RR; idx += blockDim.x) {
-                const int i = idx / R, j = idx - i * R;
-                double v = 0.0;
-                if (i != j) {
-                    const int lo = min(i, j), hi = max(i, j);
-                    v = a.m2scale * red[lo * (R - 1) - lo * (lo - 1) / 2 + (hi - lo - 1)];
-                    if (i > j) v = -v;
-                }
-                a.M2[(size_t)d * RR + idx] = v;
-            }
-            __syncthreads();
-        }
-        __threadfence_block();
-        __syncthreads();
-    }
-    if (a.do_s) {
-        // the four coefficient sets go to shared memory in one parallel load: the RK4 loops below are chains of
-        // dependent FMAs and must not wait on global memory
-        extern __shared__ double coef[];                       // [4][3 R^2]: C1, C2, D1, D2
-        const double* src[4] = {a.C1, a.C2, a.D1, a.D2};
-        for (int q = 0; q < 4; q++)
-            for (int i = threadIdx.x; i < 3 * RR; i += blockDim.x) coef[q * 3 * RR + i] = src[q][i];
-        __syncthreads();
-        dev_sflow(a.S, R, a.ts, coef, coef + 3 * RR, coef + 6 * RR, coef + 9 * RR, sc);
-        __threadfence_block();
-        __syncthreads();
-    }
-    if (a.do_tab) dev_flow_tables(a.Tm, a.lam, a.Sin, a.transS, R, a.g, a.sgn, a.tsub, a.t3, a.M2c, a.nlsign, a.o, (double*)&sc);
-}
-
-// ---------------------------------------------------------------------------------------------------------
 // column sums of a flow result from the per-CTA sums of its last pass: out[c] = sum_b part[b][c]
 __global__ void __launch_bounds__(DLR_SMALL_THREADS) k_colsum_reduce(const double* part, int nblocks, int R, double* out) {
     __shared__ double red[DLR_RMAXS], tmp[DLR_SMALL_THREADS];
     cta_reduce_rows(part, nblocks, R, 0, R, red, tmp);
     if (threadIdx.x < R) out[threadIdx.x] = red[threadIdx.x];
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// One stage of (shifted) CholeskyQR (single CTA): reduces the Gram partial sums of the producing pass itself, then
-// works entirely in shared memory (right-looking Cholesky over the whole CTA; no global loads or divisions inside
-// dependent loops).
-//   partial: [nblocks][P] upper pairs of A^T A.   stage 0 adds `shift` to the unit-diagonal scaled Gram matrix.
-//   apply[ci][co] : matrix for the next A*Mat pass (= D U^-1, times out_scale on the last stage)
-//   Rtot (row-major, upper triangular) accumulates R_stage * Rtot with R_stage = U D^-1.
-//   On the last stage the coupling matrix is written: Sout column-major = Rtot*s_scale (transS=0) or its transpose.
-//   Adaptive third stage: stage 1 holds the Gram matrix G of the once-orthogonalised factor, scaled to unit diagonal.
-//   If the Frobenius norm of its off-diagonal part is < 0.5 then ||G - I||_2 < 0.5, i.e. kappa(G) < 3 for every rank
-//   (a sufficient criterion, unlike a bound on the largest entry: a unit-diagonal Gram with all off-diagonals -1/19 is
-//   singular at r = 20), the factor after this stage is orthonormal to rounding level (CholeskyQR2 suffices for
-//   kappa(A)^2 u < 1), so stage 1 acts as the last stage and sets qrflag[0] = 1: the stage-1 A*Mat pass then writes
-//   the basis directly and the stage-2 kernels return at once.  Stage 0 clears the flag.  status[2] counts the QRs that
-//   needed the third stage.
-__global__ void __launch_bounds__(DLR_SMALL_THREADS)
-k_chol_stage(const double* partial, int nblocks, int R, int stage, int last, double shift, double out_scale,
-             double s_scale, int transS, double* apply, double* Rtot, double* Sout, int* status, int* qrflag) {
-    if (stage == 2 && qrflag[0] != 0) return;
-    __shared__ double G[DLR_RMAXS][DLR_RMAXS + 1], U[DLR_RMAXS][DLR_RMAXS + 1], Ui[DLR_RMAXS][DLR_RMAXS + 1];
-    __shared__ double Rp[DLR_RMAXS][DLR_RMAXS + 1];
-    __shared__ double dsc[DLR_RMAXS], sg[DLR_RMAXS], dinv[DLR_RMAXS];
-    __shared__ double red[DLR_RMAXS * (DLR_RMAXS + 1) / 2], tmp[DLR_SMALL_THREADS];
-    const int tid = threadIdx.x, nth = blockDim.x;
-    const int P = R * (R + 1) / 2, RR = R * R;
-    for (int idx = tid; idx < RR; idx += nth) {                 // previous Rtot (identity before the first stage)
-        const int i = idx / R, j = idx - i * R;
-        Rp[i][j] = stage ? Rtot[idx] : (i == j ? 1.0 : 0.0);
-    }
-    cta_reduce_rows(partial, nblocks, P, 0, P, red, tmp);
-    if (tid < R) {
-        const double g = red[tid * R - tid * (tid - 1) / 2];
-        dsc[tid] = g > 0.0 ? 1.0 / sqrt(g) : 1.0;
-        sg[tid] = g > 0.0 ? sqrt(g) : 1.0;
-    }
-    __syncthreads();
-    for (int idx = tid; idx < RR; idx += nth) {
-        const int i = idx / R, j = idx - i * R;
-        const int lo = min(i, j), hi = max(i, j);
-        double g = red[lo * R - lo * (lo - 1) / 2 + (hi - lo)] * dsc[i] * dsc[j];
-        if (i == j && stage == 0) g += shift;
-        G[i][j] = g;
-        U[i][j] = 0.0;
-        Ui[i][j] = 0.0;
-    }
-    __syncthreads();
-    __shared__ int s_skip;
-    if (threadIdx.x < 32) {                                     // squared Frobenius norm of the off-diagonal part
-        double f2 = 0.0;
-        for (int idx = threadIdx.x; idx < RR; idx += 32) {
-            const int i = idx / R, j = idx - i * R;
-            if (i != j) f2 = fma(G[i][j], G[i][j], f2);
-        }
-        f2 = warp_sum(f2);
-        if (threadIdx.x == 0) {
-            s_skip = (stage == 1 && f2 < 0.25) ? 1 : 0;          // NaN compares false: no skip
-            if (stage == 0) qrflag[0] = 0;
-            if (stage == 1) { qrflag[0] = s_skip; if (!s_skip) atomicAdd(status + 2, 1); }
-        }
-    }
-    __syncthreads();
-    if (s_skip) last = 1;
-    // right-looking upper Cholesky G = U^T U
-    for (int j = 0; j < R; j++) {
-        if (tid == 0) {
-            double sjj = G[j][j];
-            if (!(sjj > 1e-30)) { sjj = 1e-30; atomicAdd(status, 1); }     // repaired pivot (counted as a QR fallback)
-            double ri = rsqrt(sjj);                              // 1/sqrt(pivot), no divide/sqrt chain
-            ri = ri * fma(-0.5 * sjj * ri, ri, 1.5);               // one Newton step (rounding-level accurate)
-            U[j][j] = sjj * ri;
-            dinv[j] = ri;
-        }
-        __syncthreads();
-        if (tid > j && tid < R) U[j][tid] = G[j][tid] * dinv[j];
-        __syncthreads();
-        for (int idx = tid; idx < RR; idx += nth) {
-            const int i = idx / R, l = idx - i * R;
-            if (i > j && l >= i) G[i][l] -= U[j][i] * U[j][l];
-        }
-        __syncthreads();
-    }
-    // inverse of U (upper triangular), thread l = column l: back substitution
-    if (tid < R) {
-        const int l = tid;
-        Ui[l][l] = dinv[l];
-        for (int i = l - 1; i >= 0; i--) {
-            double sacc = 0.0;
-            for (int k = i + 1; k <= l; k++) sacc = fma(U[i][k], Ui[k][l], sacc);
-            Ui[i][l] = -sacc * dinv[i];
-        }
-    }
-    __syncthreads();
-    const double osc = last ? out_scale : 1.0;
-    for (int idx = tid; idx < RR; idx += nth) {
-        const int a = idx / R, l = idx - a * R;
-        apply[idx] = dsc[a] * Ui[a][l] * osc;
-        double sacc = 0.0;                                      // (U D^-1 Rp)[a][l], upper triangular
-        if (a <= l)
-            for (int k = a; k <= l; k++) sacc = fma(U[a][k] * sg[k], Rp[k][l], sacc);
-        Rtot[idx] = sacc;
-        if (last) {
-            if (transS) Sout[l + R * a] = sacc * s_scale;       // S = R^T
-            else Sout[a + R * l] = sacc * s_scale;              // S = R
-        }
-    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
