@@ -82,7 +82,8 @@ struct dlr_ctx {
     double *KL, *Q1, *W, *E;
     double* Em;                   // field of the diagnostics (dlr_moments): c->E stays the field used last by dlr_step
     double *partial, *partialP[3], *partialC, *partial2a;
-    double *margp1, *margp2, *margV;         // marginals of V (k_marginals partial planes; M1, M2, M3 as 3 x [r][n_v])
+    double *margp1, *margp2;                 // marginals of V: partial planes of k_marginals
+    MargOut marg;                            // M1, M2, M3 ([r][n_v] each), their DFTs and moments (k_marg_reduce)
     double *gram2, *pgram2[3], *colsum2;     // group sums of the per-CTA partial rows (group_prereduce)
     double *gramF, *pgramF[3], *colsumF;     // and their totals (one row each): what the consumers read
     unsigned* grp_cnt;                       // 3 x DLR_CNT_STRIDE group counters, zero between kernels
@@ -264,7 +265,11 @@ size_t carve(dlr_ctx* c, char* base) {
         const size_t nv = (size_t)c->gv.g.n;
         c->margp1 = cv.take<double>((size_t)R * nv * nv);
         c->margp2 = cv.take<double>((size_t)R * nv * nv);
-        c->margV = cv.take<double>(3 * (size_t)R * nv);
+        c->marg.M1 = cv.take<double>((size_t)R * nv); c->marg.M2 = cv.take<double>((size_t)R * nv);
+        c->marg.M3 = cv.take<double>((size_t)R * nv);
+        c->marg.Ph1 = cv.take<double2>((size_t)R * nv); c->marg.Ph2 = cv.take<double2>((size_t)R * nv);
+        c->marg.s0 = cv.take<double>(R); c->marg.mom3 = cv.take<double>(R);
+        c->marg.Wv = cv.take<double2>(nv);
     }
     c->partial2a = cv.take<double>((size_t)DLR_G1 * nvmax);
     const int RR = R * R;
@@ -518,8 +523,7 @@ void marginals_V(dlr_ctx* c) {
     c->count_launches -= 2;
     k_marginals<<<dim3(n, R), 256, 0, c->side>>>(c->V, hg.g, c->margp1, c->margp2);
     CK(cudaGetLastError());
-    k_marg_reduce<<<dim3(R, 3), 256, 0, c->side>>>(c->margp1, c->margp2, n, c->margV, c->margV + (size_t)R * n,
-                                         c->margV + 2 * (size_t)R * n);
+    k_marg_reduce<<<dim3(R, 3), 256, 0, c->side>>>(c->margp1, c->margp2, hg.g, c->marg);
     CK(cudaGetLastError());
     c->bytes_acc += fac_bytes(c, hg);
 }
@@ -527,12 +531,9 @@ void marginals_V(dlr_ctx* c) {
 // Column sums of the predictor's L1 (all that line 2 of Algorithm 2 needs of it) from the marginals of V and the tables
 // of the L-flow that post() has just built.
 void lpred_sums(dlr_ctx* c, double t3) {
-    const HostGrid& hg = c->gv;
-    const size_t n = (size_t)hg.g.n, R = (size_t)c->R;
-    const size_t sm = n * 16 + n * R * 16 + n * R * 8 + R * R * 8 + 8 * R * 8 + (7 * R * R + 1) * 8 + n * 16 + 64;
-    k_lpred_sums<<<1, DLR_SMALL_THREADS, sm, c->st>>>(c->margV, c->margV + R * n, c->margV + 2 * R * n, (int)R, hg.g,
-                                                      c->ft.p, t3, c->zsum);
-    CK(cudaGetLastError());
+    LpredArgs a;
+    a.m = c->marg; a.tb = c->ft.p; a.g = c->gv.g; a.t3 = t3; a.zsum = c->zsum;
+    CK(c->ops->lpred(a, c->st));
 }
 
 // The r x r work between two streaming phases, one launch (see k_post).
@@ -811,7 +812,6 @@ static cudaError_t configure_kernels(dlr_ctx* c) {
     OPTIN(k_d1<3, 3, D1_IN_CPLX, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_REAL>);
     OPTIN(k_d1<3, 3, D1_IN_REAL, D1_OP_NONE, D1_GRAM_NONE, D1_OUT_CPLX>);
     if (e == cudaSuccess) e = configure_sub2();
-    OPTIN(k_lpred_sums);
 #undef OPTIN
     return e;
 }

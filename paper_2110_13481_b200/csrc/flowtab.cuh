@@ -44,3 +44,10 @@ struct FlowTabPtrs {
     double2 *ph1, *ph2, *ez, *f1, *f2a, *f2b;   // [n][R] each, by stored (bit-reversed) position
 };
 
+// 1D marginals of V and what the flow-free predictor L step needs of them (k_marginals, k_marg_reduce -> k_lpred_sums)
+struct MargOut {
+    double *M1, *M2, *M3;        // [R][n] marginals
+    double2 *Ph1, *Ph2;          // [R][n] their DFTs (natural wavenumber order)
+    double *s0, *mom3;           // [R]
+    double2* Wv;                 // [n]
+};

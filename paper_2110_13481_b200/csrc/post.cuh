@@ -211,3 +211,112 @@ inline cudaError_t launch_post(const PostArgs& a, cudaStream_t st) {
     k_post<R><<<a.do_tab ? 5 : 1, DLR_POST_THREADS, post_smem_doubles(R) * sizeof(double), st>>>(a);
     return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// Predictor L step of Algorithm 2 without the flow.  Line 2 of Algorithm 2 needs of L1 only its column sums
+// (rho = -X (L^T omega_v), eq. (13)).  Every operation of the Lie L-flow is linear and separable:
+// the exact sub-flow along direction d preserves the marginal sums over the other directions and acts on the marginal
+// along d as the same 1D shift; the exponential-Euler stage changes the total only by t * sum_points N(m), and
+// N(m) = sum_i v_i o (m Q_i) needs the first moments sum_points v_i m only.  So the column sums of L1 follow from the three
+// 1D marginals of V (3 n r numbers), n-point DFTs and r x r products - mathematically the same numbers as the full flow.
+// The DFTs of the marginals do not depend on the coupling matrix and are done beside the coefficient passes
+// (k_marg_reduce); here only the mixing with the matrices of the L-flow (built by k_post from the predictor's S) is left:
+//   nu_d[c] = (1/n) Re sum_k ph_d[k][c] W_k sum_k' Ph_d[k'][k] B_d[k'][c],   B_1 = A0,  B_2 = A0 A1.
+// Single CTA.  zsum[c] = sum_points L1_c (no h^3 weight).
+struct LpredArgs {
+    MargOut m;
+    FlowTabPtrs tb;
+    GridDev g;
+    double t3;
+    double* zsum;
+};
+
+__host__ __device__ constexpr size_t lpred_smem_bytes(int R, int n) { return (size_t)(8 * R * R + 2 * R * n + 8 * R + 8) * 8; }
+
+template <int R>
+__global__ void __launch_bounds__(DLR_POST_THREADS) k_lpred_sums(const LpredArgs a) {
+    constexpr int RR = R * R;
+    extern __shared__ double psm[];
+    const int n = a.g.n, lg = a.g.log2n, tid = threadIdx.x, nth = blockDim.x;
+    double* msm = psm;                  // [7][RR]: A0, A1, A2, A3, Q1..3
+    double* B1 = msm + 7 * RR;          // [RR] A0 A1
+    double* parts = B1 + RR;            // [2][R][n]
+    double* vec = parts + 2 * R * n;    // 8 x [R]
+    for (int i = tid; i < 4 * RR; i += nth) msm[i] = a.tb.mats[i];
+    for (int i = tid; i < 3 * RR; i += nth) msm[4 * RR + i] = a.tb.Q[i];
+    __syncthreads();
+    const double* A0 = msm;
+    const double* A1 = msm + RR;
+    const double* A2 = msm + 2 * RR;
+    const double* A3 = msm + 3 * RR;
+    const double* Qs = msm + 4 * RR;
+    if (tid < RR) {
+        const int aa = tid / R, b = tid - aa * R;
+        double s = 0.0;
+#pragma unroll
+        for (int k = 0; k < R; k++) s = fma(A0[aa * R + k], A1[k * R + b], s);
+        B1[tid] = s;
+    }
+    __syncthreads();
+    for (int idx = tid; idx < 2 * R * n; idx += nth) {
+        const int d = idx / (R * n), e = idx - d * R * n, c = e / n, k = e - c * n;
+        const double2* Ph = (d == 0 ? a.m.Ph1 : a.m.Ph2) + k;
+        const double* B = (d == 0 ? A0 : B1) + c;
+        double2 fh = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int kk = 0; kk < R; kk++) {
+            const double2 p = Ph[(size_t)kk * n];
+            const double bb = B[kk * R];
+            fh.x = fma(p.x, bb, fh.x);
+            fh.y = fma(p.y, bb, fh.y);
+        }
+        const int ep = (int)(__brev((unsigned)k) >> (32 - lg));           // stored position of wavenumber index k
+        const double2 ph = (d == 0 ? a.tb.ph1 : a.tb.ph2)[(size_t)ep * R + c];
+        parts[idx] = cmul(cmul(ph, fh), a.m.Wv[k]).x;
+    }
+    __syncthreads();
+    double *s0 = vec, *mom3 = vec + R, *nu1 = vec + 2 * R, *nu2 = vec + 3 * R, *ta = vec + 4 * R, *tb2 = vec + 5 * R,
+           *acc = vec + 6 * R, *tmpv = vec + 7 * R;
+    {
+        const int lane = tid & 31, w = tid >> 5, nw = nth >> 5;
+        for (int row = w; row < 2 * R; row += nw) {
+            double s = 0.0;
+            for (int k = lane; k < n; k += 32) s += parts[row * n + k];
+            s = warp_sum(s);
+            if (lane == 0) (row < R ? nu1 : nu2)[row < R ? row : row - R] = s / (double)n;
+        }
+        if (tid < R) { s0[tid] = a.m.s0[tid]; mom3[tid] = a.m.mom3[tid]; }
+    }
+    __syncthreads();
+    if (tid >= 32) return;
+    // r-vector chain (row vector times matrix, [cin][cout]) by one warp
+    const auto vm = [&](const double* v, const double* Mx, double* out) {
+        double s = 0.0;
+        if (tid < R) {
+#pragma unroll
+            for (int k = 0; k < R; k++) s = fma(v[k], Mx[k * R + tid], s);
+        }
+        __syncwarp();
+        if (tid < R) out[tid] = s;
+        __syncwarp();
+    };
+    vm(s0, A0, ta); vm(ta, A1, tb2); vm(tb2, A2, acc);          // acc = sum_points m
+    vm(mom3, A0, ta); vm(ta, A1, tb2); vm(tb2, A2, mom3);       // mu_3
+    vm(nu2, A2, ta);                                            // mu_2 -> ta
+    vm(nu1, A1, tb2); vm(tb2, A2, nu1);                         // mu_1
+    if (tid < R) {
+        double gsum = 0.0;
+#pragma unroll
+        for (int k = 0; k < R; k++)
+            gsum += nu1[k] * Qs[k * R + tid] + ta[k] * Qs[RR + k * R + tid] + mom3[k] * Qs[2 * RR + k * R + tid];
+        tmpv[tid] = acc[tid] + a.t3 * gsum;
+    }
+    __syncwarp();
+    vm(tmpv, A3, a.zsum);
+}
+
+template <int R>
+inline cudaError_t launch_lpred(const LpredArgs& a, cudaStream_t st) {
+    k_lpred_sums<R><<<1, DLR_POST_THREADS, lpred_smem_bytes(R, a.g.n), st>>>(a);
+    return cudaGetLastError();
+}

@@ -36,6 +36,7 @@ struct RankOps {
     cudaError_t (*d1[V1_COUNT])(const D1Args&, cudaStream_t);
     cudaError_t (*dir[VD_COUNT])(const DirArgs&, cudaStream_t);
     cudaError_t (*post)(const PostArgs&, cudaStream_t);           // r x r work between two streaming phases (post.cuh)
+    cudaError_t (*lpred)(const LpredArgs&, cudaStream_t);         // column sums of the predictor's L1 (post.cuh)
     cudaError_t (*chol_test)(const CholArgs&, double* mat_out, cudaStream_t);     // one CholeskyQR stage on its own (test hook)
 };
 

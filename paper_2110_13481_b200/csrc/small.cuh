@@ -354,13 +354,22 @@ __global__ void __launch_bounds__(256) k_marginals(const double* A, GridDev g, d
 
 // grid (R, 3): CTA (c, which).  which 0, 1: M[c][i] = sum_k p[(c n + k) n + i] (coalesced in i, four k-groups per i);
 // which 2: M3[c][i3] = sum_i2 p2[(c n + i3) n + i2] (one warp per row, lanes along i2).
-__global__ void __launch_bounds__(256) k_marg_reduce(const double* p1, const double* p2, int n, double* M1, double* M2,
-                                                     double* M3) {
+// Then what k_lpred_sums needs of the marginals and does not depend on the coupling matrix (so it runs here, on the
+// side branch, long before the predictor's S step):  which 0, 1: Ph[c][k] = sum_i M[c][i] e^{-2 pi i ik/n} (n-point DFT
+// by its definition), which 0 also s0[c] = sum_i M1[c][i];  which 2: mom3[c] = sum_i v(i) M3[c][i], and CTA (0, 2) the
+// grid constant Wv[k] = sum_i v(i) e^{+2 pi i ik/n}.
+__global__ void __launch_bounds__(256) k_marg_reduce(const double* p1, const double* p2, GridDev g, MargOut o) {
     __shared__ double red[256];
-    const int c = blockIdx.x, which = blockIdx.y, tid = threadIdx.x;
+    __shared__ double Ms[256];
+    __shared__ double2 twf[256];
+    const int n = g.n, c = blockIdx.x, which = blockIdx.y, tid = threadIdx.x;
+    for (int m = tid; m < n; m += blockDim.x) {              // exp(-2 pi i m / n), full circle
+        const double2 w = m < (n >> 1) ? g.tw[m] : g.tw[m - (n >> 1)];
+        twf[m] = m < (n >> 1) ? w : make_double2(-w.x, -w.y);
+    }
     if (which < 2) {
         const double* p = (which == 0 ? p1 : p2) + (size_t)c * n * n;
-        double* M = (which == 0 ? M1 : M2) + (size_t)c * n;
+        double* M = (which == 0 ? o.M1 : o.M2) + (size_t)c * n;
         const int ng = max(1, (int)blockDim.x / n);              // k-groups
         for (int i0 = 0; i0 < n; i0 += blockDim.x) {
             const int i = i0 + (tid % n), kg = tid / n;
@@ -373,8 +382,24 @@ __global__ void __launch_bounds__(256) k_marg_reduce(const double* p1, const dou
                 double t = 0.0;
                 for (int gq = 0; gq < ng; gq++) t += red[gq * n + tid];
                 M[i0 + tid] = t;
+                Ms[i0 + tid] = t;
             }
             __syncthreads();
+        }
+        double2* Ph = (which == 0 ? o.Ph1 : o.Ph2) + (size_t)c * n;
+        for (int k = tid; k < n; k += blockDim.x) {
+            double2 fh = make_double2(0.0, 0.0);
+            for (int i = 0; i < n; i++) {
+                const double2 w = twf[(i * k) & (n - 1)];
+                fh.x = fma(Ms[i], w.x, fh.x);
+                fh.y = fma(Ms[i], w.y, fh.y);
+            }
+            Ph[k] = fh;
+        }
+        if (which == 0 && tid == 0) {
+            double a = 0.0;
+            for (int i = 0; i < n; i++) a += Ms[i];
+            o.s0[c] = a;
         }
     } else {
         const int lane = tid & 31, w = tid >> 5, nw = blockDim.x >> 5;
@@ -383,117 +408,25 @@ __global__ void __launch_bounds__(256) k_marg_reduce(const double* p1, const dou
             double s = 0.0;
             for (int k = lane; k < n; k += 32) s += row[k];
             s = warp_sum(s);
-            if (lane == 0) M3[(size_t)c * n + i] = s;
-        }
-    }
-}
-
-// column sums of the predictor's L1 from the marginals (see above); single CTA.  mats/Q/ph1/ph2: the tables of the
-// L-flow built by k_post (FlowTabPtrs), t3 = length of the third sub-flow.  zsum[c] = sum_points L1_c (no h^3 weight).
-__global__ void __launch_bounds__(DLR_SMALL_THREADS)
-k_lpred_sums(const double* M1, const double* M2, const double* M3, int R, GridDev g, FlowTabPtrs tb, double t3,
-             double* zsum) {
-    extern __shared__ double2 lsm[];
-    const int n = g.n, lg = g.log2n, RR = R * R, tid = threadIdx.x, nth = blockDim.x;
-    double2* W = lsm;                                   // [n]  sum_i v(i) e^{+2 pi i ik/n}
-    double2* part = W + n;                              // [n][R] terms of the moment sums
-    double* F = (double*)(part + (size_t)n * R);        // [n][R] mixed marginal
-    double* B = F + (size_t)n * R;                      // [R][R] A0 or A0 A1
-    double* vec = B + RR;                               // 8 x [R] small vectors
-    double *s0 = vec, *mom3 = vec + R, *nu1 = vec + 2 * R, *nu2 = vec + 3 * R, *ta = vec + 4 * R, *tb2 = vec + 5 * R,
-           *acc = vec + 6 * R, *tmpv = vec + 7 * R;
-    double* msm = vec + 8 * R;                          // [7][R][R]: A0, A1, A2, A3, Q1..3 (one parallel load)
-    double2* twf = (double2*)(msm + 7 * RR);             // [n] exp(-2 pi i m / n), full circle (8 R (R + 1) doubles after B: 16-byte aligned)
-    for (int i = tid; i < 4 * RR; i += nth) msm[i] = tb.mats[i];
-    for (int i = tid; i < 3 * RR; i += nth) msm[4 * RR + i] = tb.Q[i];
-    for (int m = tid; m < n; m += nth) {
-        const double2 w = m < (n >> 1) ? g.tw[m] : g.tw[m - (n >> 1)];
-        twf[m] = m < (n >> 1) ? w : make_double2(-w.x, -w.y);
-    }
-    __syncthreads();
-    const double* A0 = msm;
-    const double* A1 = msm + RR;
-    const double* A2 = msm + 2 * RR;
-    const double* A3 = msm + 3 * RR;
-    const double* Qs = msm + 4 * RR;
-    auto twd = [&](int m) { return twf[m]; };            // exp(-2 pi i m / n), 0 <= m < n
-    for (int k = tid; k < n; k += nth) {
-        double2 s = make_double2(0.0, 0.0);
-        for (int i = 0; i < n; i++) {
-            const double2 w = twd((i * k) & (n - 1));
-            const double v = g.lo + g.h * i;
-            s.x = fma(v, w.x, s.x);
-            s.y = fma(v, -w.y, s.y);                     // conjugate: e^{+...}
-        }
-        W[k] = s;
-    }
-    if (tid < R) {
-        double a = 0.0, b = 0.0;
-        for (int i = 0; i < n; i++) {
-            a += M1[(size_t)tid * n + i];
-            b = fma(g.lo + g.h * i, M3[(size_t)tid * n + i], b);
-        }
-        s0[tid] = a;
-        mom3[tid] = b;
-    }
-    __syncthreads();
-    for (int d = 0; d < 2; d++) {
-        // B = A0 (direction 1) or A0 A1 (direction 2);  F = P_d B;  nu_d[c] = (1/n) Re sum_k ph_d[k][c] F^_k[c] W_k
-        for (int idx = tid; idx < RR; idx += nth) {
-            const int a = idx / R, b = idx - a * R;
-            double s = A0[idx];
-            if (d == 1) { s = 0.0; for (int k = 0; k < R; k++) s = fma(A0[a * R + k], A1[k * R + b], s); }
-            B[idx] = s;
+            if (lane == 0) { o.M3[(size_t)c * n + i] = s; Ms[i] = s; }
         }
         __syncthreads();
-        const double* P = d == 0 ? M1 : M2;
-        for (int idx = tid; idx < n * R; idx += nth) {
-            const int i = idx / R, c = idx - i * R;
-            double s = 0.0;
-            for (int k = 0; k < R; k++) s = fma(P[(size_t)k * n + i], B[k * R + c], s);
-            F[idx] = s;
+        if (tid == 0) {
+            double b = 0.0;
+            for (int i = 0; i < n; i++) b = fma(g.lo + g.h * i, Ms[i], b);
+            o.mom3[c] = b;
         }
-        __syncthreads();
-        const double2* ph = d == 0 ? tb.ph1 : tb.ph2;
-        for (int idx = tid; idx < n * R; idx += nth) {
-            const int k = idx / R, c = idx - k * R;
-            double2 fh = make_double2(0.0, 0.0);
-            for (int i = 0; i < n; i++) {
-                const double2 w = twd((i * k) & (n - 1));
-                const double f = F[i * R + c];
-                fh.x = fma(f, w.x, fh.x);
-                fh.y = fma(f, w.y, fh.y);
+        if (c == 0) {
+            for (int k = tid; k < n; k += blockDim.x) {
+                double2 s = make_double2(0.0, 0.0);
+                for (int i = 0; i < n; i++) {
+                    const double2 wv = twf[(i * k) & (n - 1)];
+                    const double v = g.lo + g.h * i;
+                    s.x = fma(v, wv.x, s.x);
+                    s.y = fma(v, -wv.y, s.y);                     // conjugate: e^{+...}
+                }
+                o.Wv[k] = s;
             }
-            const int ep = (int)(__brev((unsigned)k) >> (32 - lg));           // stored position of wavenumber index k
-            part[idx] = cmul(cmul(ph[(size_t)ep * R + c], fh), W[k]);
         }
-        __syncthreads();
-        if (tid < R) {
-            double s = 0.0;
-            for (int k = 0; k < n; k++) s += part[k * R + tid].x;
-            (d == 0 ? nu1 : nu2)[tid] = s / (double)n;
-        }
-        __syncthreads();
     }
-    // r x r chain (row vector times matrix, [cin][cout]), by the first R threads
-    auto vm = [&](const double* v, const double* Mx, double* out) {
-        if (tid < R) {
-            double s = 0.0;
-            for (int k = 0; k < R; k++) s = fma(v[k], Mx[k * R + tid], s);
-            out[tid] = s;
-        }
-        __syncthreads();
-    };
-    vm(s0, A0, ta); vm(ta, A1, tb2); vm(tb2, A2, acc);          // acc = sum_points m
-    vm(mom3, A0, ta); vm(ta, A1, tb2); vm(tb2, A2, mom3);       // mu_3
-    vm(nu2, A2, ta);                                            // mu_2 -> ta
-    vm(nu1, A1, tb2); vm(tb2, A2, nu1);                         // mu_1
-    if (tid < R) {
-        double gsum = 0.0;
-        for (int k = 0; k < R; k++)
-            gsum += nu1[k] * Qs[k * R + tid] + ta[k] * Qs[RR + k * R + tid] + mom3[k] * Qs[2 * RR + k * R + tid];
-        tmpv[tid] = acc[tid] + t3 * gsum;
-    }
-    __syncthreads();
-    vm(tmpv, A3, zsum);
 }
