@@ -52,6 +52,7 @@ struct FlowTab {
 };
 
 struct Sub2Cfg { int L, groups, wpu, ctas; };      // launch shape of the direction-2 sub-flow (pass_sub2.cuh)
+struct Sub1Cfg { int use, NL, groups, wpu, ctas; };  // launch shape of the direction-1 sub-flow (pass_sub1.cuh); use = 0: CTA-tile kernel
 
 struct Phase {
     const char* name;
@@ -76,6 +77,7 @@ struct dlr_ctx {
     const RankOps* ops;
     HostGrid gx, gv;
     Sub2Cfg s2x, s2v;
+    Sub1Cfg s1x, s1v;
     // big buffers
     double *X, *X1, *V, *S, *Sp;     // X1: the predictor basis of Algorithm 2 (X itself stays X0 until the first K step)
     double2* Eh;
@@ -248,6 +250,7 @@ size_t carve(dlr_ctx* c, char* base) {
         size_t bd = (size_t)dir_tiles(hg->g.n, 1);            // directional tiles at L = 1 (the most there can be)
         bd = std::max(bd / hg->Lx, std::max(bd / hg->Le, bd / hg->Lc));
         blocks = std::max(blocks, std::max(b1, bd));
+        blocks = std::max(blocks, std::min((size_t)dir_tiles(hg->g.n, 1), (size_t)2048));   // persistent grids (pass_sub1.cuh)
     }
     c->partial_cap = blocks * nvmax;
     c->partial = cv.take<double>(c->partial_cap);
@@ -481,6 +484,35 @@ cudaError_t run_sub2(dlr_ctx* c, const HostGrid& hg, const double* in, double* o
     return launch_sub2(a, sc.groups, sc.ctas, c->st);
 }
 
+// sub-flow along direction 1 with both changes of basis (pass_sub1.cuh): one warp per unit of NL packed lines of all
+// columns.  Units above 48 KB (n = 256 at the larger ranks) stay with the CTA-tile kernel k_dir<r,1,EXACT>.
+void setup_sub1(dlr_ctx* c, const HostGrid& hg, Sub1Cfg& sc) {
+    const int n = hg.g.n, R = c->R;
+    sc.NL = n >= 64 ? 1 : 64 / n;
+    { const int l = tune("s1l", 0); if (is_pow2(l) && l <= n * n / 2) sc.NL = l; }
+    const size_t unit = sub1_unit_elems(n, R, sc.NL) * 16;
+    sc.wpu = unit <= 24 * 1024 ? 1 : 2;
+    { const int w = tune("s1u", 0); if (w == 1 || w == 2 || w == 4) sc.wpu = w; }
+    sc.use = unit <= 48 * 1024 && tune("s1", 1) != 0;
+    sc.groups = 8 / sc.wpu;
+    { const int w = tune("s1w", 0); if (w >= 1 && w <= 8 / sc.wpu) sc.groups = w; }
+    const size_t target = (size_t)tune("s1sm", 110) * 1024;
+    while (sc.groups > 1 && sub1_smem_bytes(n, R, sc.NL, sc.groups) > target) sc.groups--;
+    if (sub1_smem_bytes(n, R, sc.NL, sc.groups) > SMEM_MAX - 1024) sc.use = 0;
+    if (!sc.use) return;
+    const int per_sm = c->ops->sub1_occ(hg.g.log2n, sc.groups * sc.wpu * 32, sub1_smem_bytes(n, R, sc.NL, sc.groups));
+    const int units = (n * n / 2) / sc.NL;
+    sc.ctas = std::max(1, std::min(c->nsm * per_sm, (units + sc.groups - 1) / sc.groups));
+}
+cudaError_t run_sub1(dlr_ctx* c, const HostGrid& hg, const DirArgs& d) {
+    const Sub1Cfg& sc = (&hg == &c->gx) ? c->s1x : c->s1v;
+    if (!sc.use) return c->ops->dir[VD_EXACT1](d, c->st);
+    Sub1Args a;
+    a.g = hg.g; a.in = d.in; a.out = d.out; a.min_ = d.min_; a.mout = d.mout; a.ph = d.ph; a.NL = sc.NL; a.wpu = sc.wpu;
+    a.gram = d.gram; a.gram2 = d.gram2; a.gramF = d.gramF; a.grp_cnt = d.grp_cnt;
+    return c->ops->sub1(a, sc.groups, sc.ctas, c->st);
+}
+
 // Coefficient set of a factor A (N x r, real):  kind = 1: C coefficients (weights v_i, + rho_tilde);  2: D coefficients
 // (weights E_i).  Three read-only passes, one per direction: the first also accumulates the real-space weighted Gram
 // (M1 = C1 or D1, colsum), each leaves the 1D Parseval sums of its derivative coefficient in c->partialP[d] for
@@ -631,7 +663,7 @@ void flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int orde
     a.store = 1; a.L = hg.Lx;
     // sub-flow 1:  A <- src (Sin T1), phases, then into the eigenbasis of direction 2
     a.in = src; a.out = c->W; a.min_ = mats + 0 * RR; a.mout = mats + 1 * RR; a.ph = c->ft.p.ph1;
-    CK(ops->dir[VD_EXACT1](a, c->st));
+    CK(run_sub1(c, hg, a));
     c->bytes_acc += (order == 1 ? (zero_only ? 5.0 : 6.0) : 10.0) * fac_bytes(c, hg) + (is_L ? 0.0 : 24.0 * (double)hg.g.N);
     // sub-flow 2
     a.in = c->W; a.min_ = nullptr; a.mout = nullptr; a.ph = c->ft.p.ph2;
@@ -656,7 +688,7 @@ void flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int orde
     CK(ops->dir[is_L ? VD_ETD2_V : VD_ETD2_E](e, c->st));
     CK(run_sub2(c, hg, c->W, c->W, c->ft.p.ph2));                // sub-flow 2, second half
     a.out = c->KL; a.min_ = mats + 6 * RR; a.mout = mats + 7 * RR; a.ph = c->ft.p.ph1; a.gram = c->partial;
-    CK(ops->dir[VD_EXACT1](a, c->st));                           // sub-flow 1, second half, + Gram of the result
+    CK(run_sub1(c, hg, a));                                      // sub-flow 1, second half, + Gram of the result
 }
 
 // one step, issued on c->st (directly or under stream capture)
@@ -857,6 +889,8 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
     setup_sub2(c, c->gx, c->s2x);
     setup_sub2(c, c->gv, c->s2v);
+    setup_sub1(c, c->gx, c->s1x);
+    setup_sub1(c, c->gv, c->s1v);
     e = cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
@@ -1161,7 +1195,7 @@ int dlr_test_dir_pass(dlr_ctx* c, int which, int kind, const double* d_in, doubl
     if (kind < 2) {
         a.L = hg.Lx; a.ph = c->ft.p.ph1;
         if (kind == 1) CK(run_sub2(c, hg, d_in, d_out, c->ft.p.ph1));
-        else CK(c->ops->dir[VD_EXACT1](a, c->st));
+        else CK(run_sub1(c, hg, a));
     } else {
         a.threads = hg.thre; a.L = hg.Le; a.E = d_E; a.Q = c->ft.p.Q;
         a.ez = c->ft.p.ez; a.f1 = c->ft.p.f1; a.f2a = c->ft.p.f2a; a.f2b = c->ft.p.f2b;

@@ -54,8 +54,16 @@ __host__ __device__ inline int dir_zelems(int n, int LP) {
     return n * LP > need ? n * LP : need;
 }
 
+// row stride of the tile (double2 units): the point-wise phases (thread <-> (e, l), l fastest) read rows e, e+1, ... of
+// L consecutive double2 each within a quarter warp, the FFT phases consecutive lines of one row: a stride = L (mod 8)
+// puts the 8 / L rows of a quarter warp on different banks (any odd stride for L = 1, any stride for L >= 8)
+__host__ __device__ inline int dir_lpz(int lines, int L) {
+    if (L >= 8) return lines | 1;
+    return lines + (((L - lines) % 8) + 8) % 8;
+}
+
 __host__ inline size_t dir_smem_bytes(int n, int R, int L, int nbuf, int nmat, bool needE) {
-    const int LP = (nbuf * R * L) | 1;
+    const int LP = dir_lpz(nbuf * R * L, L);
     size_t b = (size_t)dir_zelems(n, LP) * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
     if (needE) b += (size_t)3 * n * L * 16;
     return b + 16;
@@ -183,7 +191,7 @@ k_dir(const DirArgs a) {
     constexpr int RR = R * R;
     const int n = a.g.n, lg = a.g.log2n, M = n >> 1, L = a.L;
     const int lL = __ffs(L) - 1;
-    const int nl = R * L, LPZ = (NBUF * nl) | 1;
+    const int nl = R * L, LPZ = dir_lpz(NBUF * nl, L);
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                        // [n][LPZ]
     double* mats = (double*)(z + dir_zelems(n, LPZ));          // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2

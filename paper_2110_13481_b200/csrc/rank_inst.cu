@@ -33,6 +33,7 @@ cudaError_t configure_rank() {
     OPTIN(k_dir<R, 2, DOP_COEFF, DW_NONE>);
     OPTIN(k_dir<R, 3, DOP_COEFF, DW_NONE>);
     OPTIN(k_post<R>);
+    if (e == cudaSuccess) e = configure_sub1<R>();
     OPTIN(k_lpred_sums<R>);
 #undef OPTIN
     return e;
@@ -61,6 +62,8 @@ extern "C" const RankOps* CAT(dlr_rank_ops_, DLR_RANK)() {
             launch_dir<R, 2, DOP_COEFF, DW_NONE>,
             launch_dir<R, 3, DOP_COEFF, DW_NONE>,
         },
+        launch_sub1<R>,
+        sub1_occupancy<R>,
         launch_post<R>,
         launch_lpred<R>,
         launch_chol_test};
