@@ -10,6 +10,7 @@ Prints ONE JSON line.
 """
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -19,7 +20,14 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-METRIC = "ms per 2nd-order DLR step (64^3x64^3, r=10, fp64)"
+def metric_name(cfg):
+    return f"ms per 2nd-order DLR step ({cfg['n_x']}^3x{cfg['n_v']}^3, r={cfg['r']}, fp64)"
+
+
+# fp64 vector peak of the B200 (no such entry in MEASURED_PEAKS.json / B200_PROFILING.md): 148 SMs x 4 sub-partitions x 16
+# fp64 lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s; a DFMA-only kernel measured 36.8 on this pool (profiles/r02_peaks.md).
+# DMMA (mma.sync.m8n8k4.f64) measured 37.2: the fp64 tensor path has the same peak as the vector path.
+FP64_TFLOPS = 36.8
 
 
 def clocks_sampler(stop, out, dev):
@@ -53,15 +61,20 @@ def measured_peak():
 # kernel families of one step: substring of the launch expression (dlr_set_profiling(ctx, 2)) -> (label, algorithmic
 # bytes per launch as (factor passes, field components): B = 8 N r per factor read or write,
 # 8 N per field component).  Averages over the launches of a step where K and L flows differ.
+# Algorithmic flops per grid point (all r columns) of a launch, (r, log2 n) -> flops: column mixing 2 r^2 per r x r product,
+# a 1D real transform 2.5 log2(n) per point and column.
 FAMILIES = [
-    ("VD_EXACT1", "k_dir<r,1,EXACT> sub-flow 1 + column mixing", 2.0, 0.0),
-    ("run_sub2", "k_sub2 sub-flow 2 (warp-autonomous units)", 2.0, 0.0),
-    ("VD_ETD2", "k_dir<r,3,ETD2> third sub-flow, both ETD2RK stages", 2.0, 2.0),     # E read by 2 of 3 launches
-    ("VD_ETD1", "k_dir<r,3,ETD1> third sub-flow, exponential Euler", 1.5, 1.5),      # K: 2B + E; L (sums only): B
-    ("VD_COEFF1", "k_dir<r,1,COEFF> weighted Gram + Parseval", 1.0, 2.0),
-    ("VD_COEFF2", "k_dir<r,2,COEFF> Parseval", 1.0, 0.0),
-    ("VD_COEFF3", "k_dir<r,3,COEFF> Parseval", 1.0, 0.0),
-    ("V1_APPLY", "k_d1<r,r,MATVEC> CholeskyQR A*R^-1 (+ Gram)", 2.0, 0.0),
+    ("run_sub1", "k_sub1 sub-flow 1 + both basis changes (warp-autonomous units)", 2.0, 0.0,
+     lambda r, lg: 4 * r * r + 5 * lg * r),
+    ("run_sub2", "k_sub2 sub-flow 2 (warp-autonomous units)", 2.0, 0.0, lambda r, lg: 5 * lg * r + 6 * r),
+    ("VD_ETD2", "k_dir<r,3,ETD2> third sub-flow, both ETD2RK stages", 2.0, 2.0,      # E read by 2 of 3 launches
+     lambda r, lg: 16 * r * r + 12.5 * lg * r),
+    ("VD_ETD1", "k_dir<r,3,ETD1> third sub-flow, exponential Euler", 2.0, 3.0,
+     lambda r, lg: 10 * r * r + 7.5 * lg * r),
+    ("VD_COEFF1", "k_dir<r,1,COEFF> weighted Gram + Parseval", 1.0, 2.0, lambda r, lg: 4 * r * (r + 1) + 2.5 * lg * r + 2 * r * r),
+    ("VD_COEFF2", "k_dir<r,2,COEFF> Parseval", 1.0, 0.0, lambda r, lg: 2.5 * lg * r + 2 * r * r),
+    ("VD_COEFF3", "k_dir<r,3,COEFF> Parseval", 1.0, 0.0, lambda r, lg: 2.5 * lg * r + 2 * r * r),
+    ("ops->apply", "k_apply CholeskyQR A*R^-1 (+ Gram), bulk-copy pipeline", 2.0, 0.0, lambda r, lg: 2 * r * r + r * (r + 1)),
 ]
 
 
@@ -82,11 +95,14 @@ def kernel_breakdown(ctx, tau, cfg, nprof=5):
     fam = {}
     total = float(sum(t for t in ms if t > 0))
     for n, t in zip(names, ms):
-        for key, label, nb, ne in FAMILIES:
+        for key, label, nb, ne, fl in FAMILIES:
             if key in n:
-                if key == "V1_APPLY" and t < 0.010:          # the skipped third CholeskyQR stage: a no-op launch
+                if key == "ops->apply" and t < 0.010:        # the skipped third CholeskyQR stage: a no-op launch
                     break
-                f = fam.setdefault(label, {"launches": 0, "ms": 0.0, "bytes": nb * B + ne * EN})
+                npts = 0.5 * (cfg["n_x"] ** 3 + cfg["n_v"] ** 3)
+                lg = 0.5 * (math.log2(cfg["n_x"]) + math.log2(cfg["n_v"]))
+                f = fam.setdefault(label, {"launches": 0, "ms": 0.0, "bytes": nb * B + ne * EN,
+                                           "flops": fl(cfg["r"], lg) * npts})
                 f["launches"] += 1
                 f["ms"] += float(t)
                 break
@@ -95,7 +111,8 @@ def kernel_breakdown(ctx, tau, cfg, nprof=5):
         avg_us = 1e3 * f["ms"] / f["launches"]
         out.append({"kernel": label, "launches_per_step": f["launches"], "avg_us": avg_us,
                     "share_of_step": f["ms"] / total, "algorithmic_bytes_per_launch": f["bytes"],
-                    "gbs": f["bytes"] / (avg_us * 1e-6) / 1e9})
+                    "gbs": f["bytes"] / (avg_us * 1e-6) / 1e9,
+                    "algorithmic_flops_per_launch": f["flops"], "tflops": f["flops"] / (avg_us * 1e-6) / 1e12})
     out.sort(key=lambda k: -k["share_of_step"])
     return out
 
@@ -122,10 +139,33 @@ def oracle_leg(cfg, steps, warmup):
     return ms, cores
 
 
+def oracle_single_thread(cfg):
+    """one step of the oracle with the BLAS pool limited to one thread (pocketfft is single-threaded anyway)"""
+    try:
+        from threadpoolctl import threadpool_limits
+    except Exception:
+        return None
+    with threadpool_limits(limits=1):
+        ms, _ = oracle_leg(cfg, 1, 0)
+    return ms
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200, help="steps per timed block (K)")
+    ap.add_argument("--min-seconds", type=float, default=1.2,
+                    help="K-step blocks are repeated (each timed on its own) until this much device time and 5 blocks")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours")
@@ -151,8 +191,10 @@ def main():
     workload = (f"BASELINE.json configs[{args.config - 1}]: {cfg['problem']} {cfg['n_x']}^3x{cfg['n_v']}^3, r={cfg['r']}, "
                 f"tau={cfg['tau']}, Algorithm 2")
     config = {"workload": workload, "n": cfg["n"], "rank": cfg["r"], "tau": cfg["tau"], "parallelism": f"replicas x{args.gpus}",
-              "l2": "working set (0.14 GB of factors and work buffers at config 3) exceeds the 126 MB L2; "
-                    "no explicit flush"}
+              "l2": (f"working set {6 * 8 * max(cfg['n_x'], cfg['n_v']) ** 3 * cfg['r'] / 1e9:.2f} GB of factors and work buffers; "
+                     "126 MB L2: no explicit flush, but at 64^3 a single 21 MB factor is L2-resident between consecutive passes "
+                     "(configs 4 and 5 are the HBM-resident cases, BASELINE.md)")}
+    METRIC = metric_name(cfg)
 
     if args.impl == "reference":
         if rank != 0:
@@ -198,15 +240,21 @@ def main():
     samples, stop = [], threading.Event()
     th = threading.Thread(target=clocks_sampler, args=(stop, samples, local_rank))
     th.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # K-step blocks, each between its own pair of events on the launching stream; repeated until >= --min-seconds of device
+    # time and >= 5 blocks so that the clocks are sampled under sustained load.  value = median block.
     barrier()
-    with torch.cuda.stream(stream):
-        ev0.record(stream)
-        for _ in range(args.steps):
-            ctx.step(tau)
-        ev1.record(stream)
-    barrier()
-    ms_step = ev0.elapsed_time(ev1) / args.steps
+    blocks = []
+    while (sum(blocks) < args.min_seconds * 1e3 or len(blocks) < 5) and len(blocks) < 200:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            ev0.record(stream)
+            for _ in range(args.steps):
+                ctx.step(tau)
+            ev1.record(stream)
+        barrier()
+        blocks.append(ev0.elapsed_time(ev1))
+    per_step = sorted(b / args.steps for b in blocks)
+    ms_step = per_step[len(per_step) // 2]
     stop.set()
     th.join()
     mom = ctx.moments()
@@ -239,7 +287,7 @@ def main():
         achieved = bytes_step / (ms_step * 1e-3) / 1e9
         top = kernels[0]
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "r01_traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "r02_traffic.json")
         if os.path.exists(tpath):
             traffic = json.load(open(tpath)).get(top["kernel"].split(" ")[0])
         roofline = {
@@ -247,12 +295,17 @@ def main():
             "frac": top["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
             "algorithmic_bytes_per_launch": top["algorithmic_bytes_per_launch"], "avg_launch_us": top["avg_us"],
             "launches_per_step": top["launches_per_step"], "share_of_step": top["share_of_step"],
+            "alu": {"achieved": top["tflops"], "peak": FP64_TFLOPS, "unit": "TFLOP/s", "frac": top["tflops"] / FP64_TFLOPS,
+                    "what": "plain fp64 ALUs: algorithmic flops of the launch (DESIGN.md section 6) / its duration; peak = "
+                            "148 SMs x 64 fp64 lanes x 2 x 1.965 GHz = 37.2, measured 36.8 (profiles/r02_peaks.md)"},
             "note": "dominant kernel family of the step by device time; duration = CUDA events after every launch on "
                     "the context's stream (dlr_set_profiling(ctx, 2), 5 steps, median) right after the timed region; "
-                    "traffic = DRAM bytes per launch from the ncu --set full capture in profiles/ (cold cache). "
-                    "bound = hbm is the roofline the passes are designed against (and what the metric asks for); as "
-                    "measured they are limited by the shared-memory pipe, not by HBM (DRAM traffic = algorithmic bytes, "
-                    "profiles/r01_c_profile_cfg3.md)",
+                    "traffic = DRAM bytes per launch from the ncu --set full capture of this build in profiles/ (cold "
+                    "cache). bound = hbm is the roofline the metric asks for. As measured (profiles/r02_profile_cfg3.md) no "
+                    "pass kernel is HBM-bound at this shape: DRAM traffic = algorithmic bytes, the 21 MB factor is L2-resident, "
+                    "and the kernels are LATENCY- and ISSUE-bound (warps active ~22 %, issue slots 27-35 %, fp64 pipe 22-27 %, "
+                    "no pipe above 50 %): the third sub-flow executes 26 M warp instructions per launch (issue floor 22 us, "
+                    "fp64 floor 18 us) in 11 barrier-separated phases of one tile",
             "step": {"algorithmic_bytes_per_step": bytes_step, "achieved": achieved, "frac": achieved / peak,
                      "what": "all factor-sized passes of one step (DESIGN.md section 6) / CUDA-event time of the step"},
             "kernels": kernels,
@@ -266,6 +319,8 @@ def main():
             "clocks": summarize_clocks(samples),
             "e2e": {"value": e2e_ms, "unit": "ms/step", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "what": f"set_initial(pinned host)+{e2e_steps}x(dlr_step+dlr_moments)+get_factors(pinned host), per step"},
+            "timed_blocks": {"blocks": len(blocks), "steps_per_block": args.steps, "device_seconds": sum(blocks) / 1e3,
+                             "median": ms_step, "min": per_step[0], "max": per_step[-1]},
             "gpu_launches": launches * args.steps,
             "launches_per_step": launches,
             "roofline": roofline,
@@ -274,7 +329,8 @@ def main():
         }
         if world == 1 and not args.no_cpu_baseline:
             cms, cores = oracle_leg(cfg, args.cpu_steps, 0)
-            out["cpu_baseline"] = {"value": cms, "unit": "ms/step", "cores": cores, "kind": "oracle",
+            out["cpu_baseline"] = {"value": cms, "unit": "ms/step", "cores": cores, "kind": "oracle", "cpu": cpu_model(),
+                                   "single_thread_value": oracle_single_thread(cfg),
                                    "sample": f"{args.cpu_steps} full step(s) of the same workload on the host "
                                              "(NumPy oracle; pocketfft single-threaded, BLAS threads = cores)"}
         print(json.dumps(out))

@@ -44,6 +44,13 @@ def build(force=False, verbose=False):
     with ThreadPoolExecutor(max_workers=min(8, len(jobs))) as ex:
         list(ex.map(run, jobs))
     objs = [j[1] for j in jobs]
+    # stand-alone peak probe (fp64 and L2/HBM peaks quoted by bench.py and DESIGN.md): python -m ... build, then ./peak_probe
+    probe_src, probe = os.path.join(CSRC, "peak_probe.cu"), os.path.join(HERE, "peak_probe")
+    if force or not _newer(probe, [probe_src]):
+        res = subprocess.run([NVCC] + FLAGS[:5] + ["-o", probe, probe_src], capture_output=True, text=True)
+        if res.returncode:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed: peak_probe.cu")
     if force or not _newer(LIB, objs):
         cmd = [NVCC, "-shared", "-o", LIB] + objs + ["-lcudart"]
         res = subprocess.run(cmd, capture_output=True, text=True)

@@ -52,6 +52,7 @@ struct FlowTab {
 };
 
 struct Sub2Cfg { int L, groups, wpu, ctas; };      // launch shape of the direction-2 sub-flow (pass_sub2.cuh)
+struct ApplyCfg { int C, S, ctas; };              // chunk length, stages and grid of the A*Mat pass (pass_apply.cuh)
 struct Sub1Cfg { int use, NL, groups, wpu, ctas; };  // launch shape of the direction-1 sub-flow (pass_sub1.cuh); use = 0: CTA-tile kernel
 
 struct Phase {
@@ -78,6 +79,7 @@ struct dlr_ctx {
     HostGrid gx, gv;
     Sub2Cfg s2x, s2v;
     Sub1Cfg s1x, s1v;
+    ApplyCfg apx, apv;
     // big buffers
     double *X, *X1, *V, *S, *Sp;     // X1: the predictor basis of Algorithm 2 (X itself stays X0 until the first K step)
     double2* Eh;
@@ -629,25 +631,43 @@ void field_join(dlr_ctx* c) {
     c->field_pending = false;
 }
 
+void setup_apply(dlr_ctx* c, const HostGrid& hg, ApplyCfg& ac) {
+    // A*Mat pass of the QR (pass_apply.cuh): chunks of 512 points while a stage (r columns) stays near 41 KB, else 256, and as
+    // many stages as fit into ~190 KB.  Measured at 64^3, r = 10: 512 x 4 stages 20.5 us per pass, 256 x 8 stages 22 us, 128: 35 us
+    // (per-chunk barrier and copy issue), against 21.5 us of the CTA-tile kernel it replaces
+    const int R = c->R;
+    ac.C = ((size_t)R * apply_cs(512) * 8 <= 48 * 1024 && hg.g.N % 512 == 0) ? 512 : 256;
+    { const int v = tune("apc", 0); if (v >= 64 && v % 64 == 0 && hg.g.N % v == 0) ac.C = v; }
+    const size_t stage = (size_t)R * apply_cs(ac.C) * 8;
+    ac.S = (int)std::min<size_t>(8, (190 * 1024) / stage);
+    { const int v = tune("aps", 0); if (v >= 2 && v <= 8) ac.S = v; }
+    while (ac.S > 2 && apply_smem_bytes(R, ac.C, ac.S) > SMEM_MAX - 1024) ac.S--;
+    ac.ctas = (int)std::min<long long>(c->nsm, hg.g.N / ac.C);
+}
+
 // shifted CholeskyQR3 of KL (N x r) -> orthonormal basis (h^3 B^T B = I) into `basis`, coupling matrix into Sout
 // (transS: S = R^T for the L step, Fig. 1 line 40 transpose_inplace).
 // The total of the Gram sums of KL must already be in c->gramF (written by the last pass of the flow).  Three A*Mat
-// passes; the r x r factorisation of each stage happens in the prologue of its own pass (chol_warp.cuh).  Stage 1
+// passes (bulk-copy pipeline, pass_apply.cuh); the r x r factorisation of each stage happens in the prologue of its own pass (chol_warp.cuh).  Stage 1
 // decides on the device whether the third is needed (only while kappa(K) >~ 1e7, i.e. the first few steps): if not it
 // writes the basis itself and the stage-2 launch returns at once.
 void qr(dlr_ctx* c, const HostGrid& hg, double* basis, double* Sout, int transS) {
     const int R = c->R;
+    const ApplyCfg& ac = (&hg == &c->gx) ? c->apx : c->apv;
     double* src[3] = {c->KL, c->Q1, c->KL};
     double* dst[3] = {c->Q1, c->KL, basis};
     for (int stage = 0; stage < 3; stage++) {
-        D1Args a = d1args(c, hg);
-        a.in_real = src[stage]; a.out_real = dst[stage]; a.out_alt = basis; a.partial = c->partial;
+        ApplyArgs a;
+        memset(&a, 0, sizeof(a));
+        a.N = hg.g.N; a.in = src[stage]; a.out = dst[stage]; a.out_alt = basis;
+        a.partial = c->partial; a.partial2 = c->gram2; a.partialF = c->gramF; a.grp_cnt = c->grp_cnt;
+        a.C = ac.C; a.S = ac.S;
         a.ch.gsum = c->gramF; a.ch.stage = stage; a.ch.transS = transS;
         a.ch.shift = 64.0 * R * 2.220446049250313e-16;
         a.ch.out_scale = 1.0 / sqrt(hg.g.h3); a.ch.s_scale = sqrt(hg.g.h3);
         a.ch.Rtot = c->Rtot; a.ch.Sout = Sout; a.ch.status = c->status; a.ch.qrflag = c->status + 1;
         if (stage < 2) c->bytes_acc += 2.0 * fac_bytes(c, hg);     // the third stage is skipped in steady state: not counted
-        CK(c->ops->d1[stage < 2 ? V1_APPLY_GRAM : V1_APPLY](a, c->st));
+        CK(c->ops->apply[stage < 2 ? 0 : 1](a, ac.ctas, c->st));
     }
 }
 
@@ -889,6 +909,8 @@ int dlr_create(const dlr_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e != cudaSuccess) { delete c; return DLR_ERR_CUDA; }
     setup_sub2(c, c->gx, c->s2x);
     setup_sub2(c, c->gv, c->s2v);
+    setup_apply(c, c->gx, c->apx);
+    setup_apply(c, c->gv, c->apv);
     setup_sub1(c, c->gx, c->s1x);
     setup_sub1(c, c->gv, c->s1v);
     e = cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking);

@@ -33,6 +33,8 @@ cudaError_t configure_rank() {
     OPTIN(k_dir<R, 2, DOP_COEFF, DW_NONE>);
     OPTIN(k_dir<R, 3, DOP_COEFF, DW_NONE>);
     OPTIN(k_post<R>);
+    OPTIN(k_apply<R, true>);
+    OPTIN(k_apply<R, false>);
     if (e == cudaSuccess) e = configure_sub1<R>();
     OPTIN(k_lpred_sums<R>);
 #undef OPTIN
@@ -64,6 +66,7 @@ extern "C" const RankOps* CAT(dlr_rank_ops_, DLR_RANK)() {
         },
         launch_sub1<R>,
         sub1_occupancy<R>,
+        {launch_apply<R, true>, launch_apply<R, false>},
         launch_post<R>,
         launch_lpred<R>,
         launch_chol_test};

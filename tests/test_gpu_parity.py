@@ -245,7 +245,12 @@ def test_config5_one_step_golden():
 def test_predictor_L_shortcut_equals_the_flow():
     """the predictor of Algorithm 2 takes rho(L^1) from the 1D marginals of V instead of running the L flow (DESIGN.md
     row a7').  A/B against the literal flow (DLR_FLAG_PREDICTOR_L_FLOW) after several steps, when S has full rank and
-    the field is nonlinear (alpha = 0.5): E^{1/2} point-wise and f at the probes."""
+    the field is nonlinear (alpha = 0.5): E^{1/2} point-wise (what the shortcut produces) to 1e-11, f at the probes to 1e-10.
+    The bound on f is north_star's one-step tolerance, not 1e-11: at 128^3, r = 15 this configuration amplifies rounding by
+    ~1e5 through the ill-conditioned first QRs - two builds of the SAME algorithm that differ only in summation order (the
+    CTA-tile and the warp-autonomous sub-flow-1 kernel) differ by 3-6e-11 in f after these 3 steps and by 1.9e-10 in
+    E^{1/2} after one, while shortcut and flow agree to 1.5e-15 in E^{1/2} after one step and 8e-13 after three (measured
+    on B200, reading R18)."""
     from paper_2110_13481_b200 import dlr
     for n, r, nsteps in ((64, 10, 6), (128, 15, 3)):
         cfg = inputs.make_config(4, n_x=n, n_v=n, r=r)
@@ -261,7 +266,7 @@ def test_predictor_L_shortcut_equals_the_flow():
             ctx.close()
         (Ea, fa, ma), (Eb, fb, mb) = res
         assert np.abs(Ea - Eb).max() <= 1e-11 * np.abs(Eb).max(), (n, r)
-        assert np.abs(fa - fb).max() <= 1e-11 * np.abs(fb).max(), (n, r)
+        assert np.abs(fa - fb).max() <= 1e-10 * np.abs(fb).max(), (n, r)
         assert rel(ma["electric_energy"], mb["electric_energy"]) <= 1e-11
 
 
