@@ -321,6 +321,8 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     hg.T1s = choose_T1(n, 3, false, 4);
     hg.T3 = choose_T3(n, R, 4 * R * R);
     hg.T3s = choose_T3(n, 3, 0);
+    { const int v = tune("t1s", 0); if (is_pow2(v) && v <= n * n) hg.T1s = v; }
+    { const int v = tune("t3s", 0); if (is_pow2(v) && v <= 16) hg.T3s = v; }
     const int t1 = tune("t1", 0), t3 = tune("t3", 0);
     if (is_pow2(t1) && t1 <= n * n && d1_smem_bytes(n, R, t1, true, 3 * R * R) <= SMEM_MAX) hg.T1 = t1;
     if (is_pow2(t3) && t3 <= 16 && d3_smem_bytes(n, R, t3, 4 * R * R) <= SMEM_MAX) hg.T3 = t3;
@@ -330,7 +332,9 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     hg.thr3 = valid_threads(tune("thr3", DLR_THREADS));
     auto dthreads = [](int t) { return (t >= 64 && t <= DLR_THREADS && t % 32 == 0) ? t : DLR_THREADS; };
     hg.thrx = dthreads(tune("thrx", DLR_THREADS));
-    hg.thre = dthreads(tune("thre", DLR_THREADS));
+    // third sub-flow above rank 10: one CTA per SM (register budget), so 512 threads (128 registers each) instead of 256
+    { const int t = tune("thre", R > 10 ? 2 * DLR_THREADS : DLR_THREADS);
+      hg.thre = (t >= 64 && t <= (R > 10 ? 2 : 1) * DLR_THREADS && t % 32 == 0) ? t : DLR_THREADS; }
     { const int t = tune("thrx2", 0); hg.thrx2 = (t >= 64 && t <= 2 * DLR_THREADS && t % 32 == 0) ? t : 0; }
     hg.thrc = dthreads(tune("thrc", DLR_THREADS));
     const int lmax = 8;

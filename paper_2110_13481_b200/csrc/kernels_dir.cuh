@@ -177,7 +177,7 @@ __device__ __forceinline__ void tp_decode(int tp, int& I, int& J) {
 }
 
 template <int R, int DIR, int DOP, int DW>
-__global__ void __launch_bounds__((DOP == DOP_EXACT && DIR == 2) ? 2 * DLR_THREADS : DLR_THREADS,
+__global__ void __launch_bounds__(((DOP == DOP_EXACT && DIR == 2) || ((DOP == DOP_ETD1 || DOP == DOP_ETD2) && R > 10)) ? 2 * DLR_THREADS : DLR_THREADS,
                                   ((DOP == DOP_EXACT && DIR == 2) ? (R <= 10 ? 2 : 1)
                                    : (DOP == DOP_COEFF && DW == DW_NONE) ? (R <= 10 ? 3 : (R <= 16 ? 2 : 1))
                                    : (DOP == DOP_COEFF || DOP == DOP_EXACT) ? (R <= 16 ? 2 : 1)
