@@ -54,6 +54,11 @@ __host__ __device__ inline int dir_zelems(int n, int LP) {
     return n * LP > need ? n * LP : need;
 }
 
+// r x r matrices in shared memory: row stride padded to an even number of doubles so that the coefficients of two
+// neighbouring output columns come with ONE 128-bit load (one LDS per four FMAs instead of one per two)
+__host__ __device__ constexpr int mat_rs(int R) { return (R + 1) & ~1; }
+__host__ __device__ constexpr int mat_ms(int R) { return R * mat_rs(R); }
+
 // row stride of the tile (double2 units): the point-wise phases (thread <-> (e, l), l fastest) read rows e, e+1, ... of
 // L consecutive double2 each within a quarter warp, the FFT phases consecutive lines of one row: a stride = L (mod 8)
 // puts the 8 / L rows of a quarter warp on different banks (any odd stride for L = 1, any stride for L >= 8)
@@ -64,7 +69,7 @@ __host__ __device__ inline int dir_lpz(int lines, int L) {
 
 __host__ inline size_t dir_smem_bytes(int n, int R, int L, int nbuf, int nmat, bool needE) {
     const int LP = dir_lpz(nbuf * R * L, L);
-    size_t b = (size_t)dir_zelems(n, LP) * 16 + (size_t)((nmat * R * R + 1) & ~1) * 8;
+    size_t b = (size_t)dir_zelems(n, LP) * 16 + (size_t)nmat * mat_ms(R) * 8;
     if (needE) b += (size_t)3 * n * L * 16;
     return b + 16;
 }
@@ -112,58 +117,80 @@ __device__ __forceinline__ void dir_weights(const DirGeom& gm, const double2* Et
     }
 }
 
+// copy a dense [R][R] matrix into the padded layout (pads zeroed); all threads of the CTA
 template <int R>
-__device__ __forceinline__ void dir_matvec(double2 (&x)[R], const double* A) {     // x <- x * A, A[cin][cout]
+__device__ __forceinline__ void mat_stage(double* dst, const double* __restrict__ src) {
+    constexpr int RS = mat_rs(R);
+    for (int i = threadIdx.x; i < R * RS; i += blockDim.x) {
+        const int ci = i / RS, co = i - ci * RS;
+        dst[i] = co < R ? src[ci * R + co] : 0.0;
+    }
+}
+
+template <int R>
+__device__ __forceinline__ void dir_matvec(double2 (&x)[R], const double* A) {     // x <- x * A, A[cin][cout] (padded)
+    constexpr int RS = mat_rs(R);
     double2 y[R];
 #pragma unroll
-    for (int co = 0; co < R; co++) {
-        double2 acc = make_double2(0.0, 0.0);
+    for (int co = 0; co < R; co += 2) {
+        double2 a0 = make_double2(0.0, 0.0), a1 = a0;
 #pragma unroll
         for (int ci = 0; ci < R; ci++) {
-            const double m = A[ci * R + co];
-            acc.x = fma(m, x[ci].x, acc.x);
-            acc.y = fma(m, x[ci].y, acc.y);
+            const double2 m = *(const double2*)(A + ci * RS + co);
+            a0.x = fma(m.x, x[ci].x, a0.x); a0.y = fma(m.x, x[ci].y, a0.y);
+            a1.x = fma(m.y, x[ci].x, a1.x); a1.y = fma(m.y, x[ci].y, a1.y);
         }
-        y[co] = acc;
+        y[co] = a0;
+        if (co + 1 < R) y[co + 1] = a1;
     }
 #pragma unroll
     for (int c = 0; c < R; c++) x[c] = y[c];
 }
 
-// out[co * stride] = (x A)[co], streamed out one component at a time (x is fully in registers, so out may alias the
+// out[co * stride] = (x A)[co], streamed out two components at a time (x is fully in registers, so out may alias the
 // place x was loaded from): no second r-vector in registers
 template <int R>
 __device__ __forceinline__ void dir_matvec_store(const double2 (&x)[R], const double* A, double2* out, int stride) {
+    constexpr int RS = mat_rs(R);
 #pragma unroll
-    for (int co = 0; co < R; co++) {
-        double2 acc = make_double2(0.0, 0.0);
+    for (int co = 0; co < R; co += 2) {
+        double2 a0 = make_double2(0.0, 0.0), a1 = a0;
 #pragma unroll
         for (int ci = 0; ci < R; ci++) {
-            const double m = A[ci * R + co];
-            acc.x = fma(m, x[ci].x, acc.x);
-            acc.y = fma(m, x[ci].y, acc.y);
+            const double2 m = *(const double2*)(A + ci * RS + co);
+            a0.x = fma(m.x, x[ci].x, a0.x); a0.y = fma(m.x, x[ci].y, a0.y);
+            a1.x = fma(m.y, x[ci].x, a1.x); a1.y = fma(m.y, x[ci].y, a1.y);
         }
-        out[co * stride] = acc;
+        out[co * stride] = a0;
+        if (co + 1 < R) out[(co + 1) * stride] = a1;
     }
 }
 
 // real-space term in the eigenbasis: g = sum_i w_i o (m Q_i), component co written to gout[co * stride]
-// (streamed out one component at a time: only m stays in registers)
+// (streamed out two components at a time: only m stays in registers); Q = three padded matrices
 template <int R>
 __device__ __forceinline__ void dir_nonlin(const double2 (&m)[R], double2* gout, int stride, const double* Q, double2 w0,
                                            double2 w1, double2 w2) {
+    constexpr int RS = mat_rs(R), MS = mat_ms(R);
 #pragma unroll
-    for (int co = 0; co < R; co++) {
-        double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
+    for (int co = 0; co < R; co += 2) {
+        double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0, t0 = s0, t1 = s0, t2 = s0;
 #pragma unroll
         for (int ci = 0; ci < R; ci++) {
-            const double q0 = Q[ci * R + co], q1 = Q[R * R + ci * R + co], q2 = Q[2 * R * R + ci * R + co];
-            s0.x = fma(q0, m[ci].x, s0.x); s0.y = fma(q0, m[ci].y, s0.y);
-            s1.x = fma(q1, m[ci].x, s1.x); s1.y = fma(q1, m[ci].y, s1.y);
-            s2.x = fma(q2, m[ci].x, s2.x); s2.y = fma(q2, m[ci].y, s2.y);
+            const double2 q0 = *(const double2*)(Q + ci * RS + co), q1 = *(const double2*)(Q + MS + ci * RS + co),
+                          q2 = *(const double2*)(Q + 2 * MS + ci * RS + co);
+            s0.x = fma(q0.x, m[ci].x, s0.x); s0.y = fma(q0.x, m[ci].y, s0.y);
+            s1.x = fma(q1.x, m[ci].x, s1.x); s1.y = fma(q1.x, m[ci].y, s1.y);
+            s2.x = fma(q2.x, m[ci].x, s2.x); s2.y = fma(q2.x, m[ci].y, s2.y);
+            t0.x = fma(q0.y, m[ci].x, t0.x); t0.y = fma(q0.y, m[ci].y, t0.y);
+            t1.x = fma(q1.y, m[ci].x, t1.x); t1.y = fma(q1.y, m[ci].y, t1.y);
+            t2.x = fma(q2.y, m[ci].x, t2.x); t2.y = fma(q2.y, m[ci].y, t2.y);
         }
         gout[co * stride] = make_double2(fma(w0.x, s0.x, fma(w1.x, s1.x, w2.x * s2.x)),
                                          fma(w0.y, s0.y, fma(w1.y, s1.y, w2.y * s2.y)));
+        if (co + 1 < R)
+            gout[(co + 1) * stride] = make_double2(fma(w0.x, t0.x, fma(w1.x, t1.x, w2.x * t2.x)),
+                                                   fma(w0.y, t0.y, fma(w1.y, t1.y, w2.y * t2.y)));
     }
 }
 
@@ -188,14 +215,14 @@ k_dir(const DirArgs a) {
                                                                   // direction-2 sub-flow keeps a small register budget
     constexpr int NBUF = ETD ? 2 : 1;
     constexpr int NMAT = ETD ? 5 : 2;
-    constexpr int RR = R * R;
+    constexpr int MS = mat_ms(R);
     const int n = a.g.n, lg = a.g.log2n, M = n >> 1, L = a.L;
     const int lL = __ffs(L) - 1;
     const int nl = R * L, LPZ = dir_lpz(NBUF * nl, L);
     extern __shared__ double2 smem2[];
     double2* z = smem2;                                        // [n][LPZ]
-    double* mats = (double*)(z + dir_zelems(n, LPZ));          // [NMAT][R*R]: Min, Mout, Q0, Q1, Q2
-    double2* Et = (double2*)(mats + ((NMAT * RR + 1) & ~1));   // [3][n][L]
+    double* mats = (double*)(z + dir_zelems(n, LPZ));          // [NMAT] padded matrices: Min, Mout, Q0, Q1, Q2
+    double2* Et = (double2*)(mats + NMAT * MS);                // [3][n][L]
     const int tid = threadIdx.x, nth = blockDim.x;
     DirGeom gm;
     gm.n = n; gm.lg = lg; gm.M = M; gm.L = L; gm.lL = lL; gm.lo = a.g.lo; gm.h = a.g.h;
@@ -207,9 +234,9 @@ k_dir(const DirArgs a) {
         gm.ia = (int)blockIdx.x >> ltp;
         gm.j0 = ((int)blockIdx.x & ((1 << ltp) - 1)) << lL;
     }
-    if (MIX && a.min_ != nullptr) for (int i = tid; i < RR; i += nth) mats[i] = a.min_[i];
-    if (MIX && a.mout != nullptr) for (int i = tid; i < RR; i += nth) mats[RR + i] = a.mout[i];
-    if (ETD) for (int i = tid; i < 3 * RR; i += nth) mats[2 * RR + i] = a.Q[i];
+    if (MIX && a.min_ != nullptr) mat_stage<R>(mats, a.min_);
+    if (MIX && a.mout != nullptr) mat_stage<R>(mats + MS, a.mout);
+    if (ETD) { mat_stage<R>(mats + 2 * MS, a.Q); mat_stage<R>(mats + 3 * MS, a.Q + R * R); mat_stage<R>(mats + 4 * MS, a.Q + 2 * R * R); }
     const size_t N2 = (size_t)(a.g.N >> 1);
     const double invn = 1.0 / (double)n;
 
@@ -367,7 +394,7 @@ k_dir(const DirArgs a) {
                 double2 x[R];
 #pragma unroll
                 for (int c = 0; c < R; c++) x[c] = p[c * L];
-                dir_matvec_store<R>(x, mats + RR, p, L);
+                dir_matvec_store<R>(x, mats + MS, p, L);
             }
             __syncthreads();
         }
@@ -375,7 +402,7 @@ k_dir(const DirArgs a) {
 
     if (ETD) {
         // -------------------------------------------------------------- third sub-flow, exponential Runge-Kutta
-        const double* Q = mats + 2 * RR;
+        const double* Q = mats + 2 * MS;
         for (int w = tid; w < pitems; w += nth) {             // m = A Min,  g0 = N'(m)
             const int l = w & (L - 1), e = w >> lL;
             double2* p = z + (size_t)e * LPZ + l;
@@ -434,7 +461,7 @@ k_dir(const DirArgs a) {
             double2 x[R];
 #pragma unroll
             for (int c = 0; c < R; c++) { x[c] = p[c * L]; x[c].x *= invn; x[c].y *= invn; }
-            if (a.mout != nullptr) dir_matvec<R>(x, mats + RR);
+            if (a.mout != nullptr) dir_matvec<R>(x, mats + MS);
 #pragma unroll
             for (int c = 0; c < R; c++) p[c * L] = x[c];
         }

@@ -36,7 +36,7 @@ __host__ inline size_t sub1_smem_bytes(int n, int R, int NL, int groups) {
     size_t units = sub1_unit_elems(n, R, NL) * groups;
     const size_t need = (size_t)groups * 8 * 64 / 2;          // scratch of the cross-warp MMA reduction (8 warps max per group set)
     if (units < need) units = need;
-    return ((size_t)p.tlen + (size_t)n * sub1_rp(R) + (size_t)((2 * R * R + 1) & ~1) / 2 + 1 + units) * 16;
+    return ((size_t)p.tlen + (size_t)n * sub1_rp(R) + (size_t)(2 * mat_ms(R)) / 2 + 1 + units) * 16;
 }
 
 template <int R, int LG>
@@ -44,13 +44,13 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
     extern __shared__ double2 smem2[];
     constexpr int n = 1 << LG, lg = LG;
     constexpr WPlan p = wf_plan(LG);
-    constexpr int RR = R * R, RP = sub1_rp(R);
+    constexpr int MS = mat_ms(R), RP = sub1_rp(R);
     constexpr int NTP = GramShape<R>::NTP, NB = GramShape<R>::NB;
     const int NL = a.NL, lNL = __ffs(NL) - 1;
     double2* tab = smem2;                                   // twiddle tables
     double2* phs = tab + p.tlen;                            // [n][RP] phases times 1/n
     double* mats = (double*)(phs + n * RP);                 // Min, Mout
-    double2* zbase = (double2*)(mats + ((2 * RR + 1) & ~1)) + 1;
+    double2* zbase = (double2*)(mats + 2 * MS) + 1;
     const int gsz = a.wpu << 5;
     const int grp = (int)threadIdx.x / gsz, ngrp = (int)blockDim.x / gsz;
     ZL zl;
@@ -64,8 +64,8 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
         phs[e * RP + c] = make_double2(f.x * invn, f.y * invn);
     }
     const bool has_min = a.min_ != nullptr, has_mout = a.mout != nullptr;
-    if (has_min) for (int i = threadIdx.x; i < RR; i += blockDim.x) mats[i] = a.min_[i];
-    if (has_mout) for (int i = threadIdx.x; i < RR; i += blockDim.x) mats[RR + i] = a.mout[i];
+    if (has_min) mat_stage<R>(mats, a.min_);
+    if (has_mout) mat_stage<R>(mats + MS, a.mout);
     __syncthreads();
     Grp gp;
     gp.tid = (int)threadIdx.x - grp * gsz; gp.nth = gsz; gp.bar = 1 + grp;
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
                 const double2* pp = phs + e * RP;
 #pragma unroll
                 for (int c = 0; c < R; c++) x[c] = cmul(x[c], pp[c]);
-                if (has_mout) dir_matvec_store<R>(x, mats + RR, pz, zl.CP);
+                if (has_mout) dir_matvec_store<R>(x, mats + MS, pz, zl.CP);
                 else {
 #pragma unroll
                     for (int c = 0; c < R; c++) pz[c * zl.CP] = x[c];
