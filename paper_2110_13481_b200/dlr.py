@@ -115,7 +115,8 @@ def _ptr(a):
 class Dlr:
     """One context = one simulation on one GPU/stream.  Methods are the C calls with the `dlr_` prefix dropped."""
 
-    def __init__(self, cfg, device="cuda:0", stream=None):
+    def __init__(self, cfg, device="cuda:0", stream=None, guard_bytes=0):
+        """guard_bytes > 0 puts that many pattern bytes before and after the workspace (check_guards(): tests only)"""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the DLR hot path has no CPU fallback")
@@ -127,15 +128,22 @@ class Dlr:
         self.Nv = cfg.n_v[0] * cfg.n_v[1] * cfg.n_v[2]
         nbytes = dlr_workspace_bytes(cfg)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.workspace = torch.full((nbytes + 512 + 2 * guard_bytes,), 0xA5, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         base = self.workspace.data_ptr()
-        self._ws_ptr = (base + 255) // 256 * 256
+        self._ws_ptr = (base + guard_bytes + 255) // 256 * 256
+        self._guards = (self._ws_ptr - base, self._ws_ptr - base + nbytes) if guard_bytes else None
         h = ctypes.c_void_p()
         rc = lib().dlr_create(ctypes.byref(cfg), self._ws_ptr, nbytes, self.stream.cuda_stream, ctypes.byref(h))
         if rc != DLR_OK:
             raise DlrError(rc, "dlr_create")
         self.h = h
+
+    def check_guards(self):
+        """True if no byte outside [workspace, workspace + dlr_workspace_bytes) was written since creation"""
+        lo, hi = self._guards
+        self.torch.cuda.synchronize(self.device)
+        return bool((self.workspace[:lo] == 0xA5).all().item()) and bool((self.workspace[hi:] == 0xA5).all().item())
 
     def _check(self, rc, where):
         if rc != DLR_OK:

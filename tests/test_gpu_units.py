@@ -316,3 +316,25 @@ def test_rank_deficient_factor_in_the_qr(case):
         # COUNTED, the state stays finite and f stays 0; the caller sees qr_fallbacks > 0
         assert m["qr_fallbacks"] > 0
     ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n_x,n_v,r,order", [(8, 8, 5, 2), (16, 16, 10, 2), (16, 16, 15, 1), (8, 32, 8, 2), (32, 16, 20, 2),
+                                             (64, 64, 10, 2), (64, 32, 15, 2), (128, 8, 10, 2)])
+def test_nothing_is_written_outside_the_workspace(n_x, n_v, r, order):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so out-of-bounds writes are looked for with
+    guard bands: 1 MiB of pattern bytes directly before and after the caller-owned workspace must survive steps (direct
+    launch and graph replay), diagnostics and a factor read-out at tile shapes from n = 8 to 128 and all ranks."""
+    from paper_2110_13481_b200 import dlr
+    cfg = inputs.make_config(1, n_x=n_x, n_v=n_v, r=r)
+    X, S, V = inputs.initial_factors(cfg)
+    ix, iv = inputs.probe_indices(cfg)
+    ctx = dlr.Dlr(dlr.config_from_inputs(cfg, order=order), device="cuda:0", guard_bytes=1 << 20)
+    ctx.set_initial(X, S, V)
+    ctx.run(cfg["tau"], 3)
+    m, f = ctx.moments(ix, iv)
+    ctx.get_factors()
+    ctx.get_field()
+    assert np.isfinite(f).all() and m["nonfinite"] == 0
+    assert ctx.check_guards()
+    ctx.close()
