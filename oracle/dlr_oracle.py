@@ -10,7 +10,9 @@ Cassini & Einkemmer, arXiv 2110.13481 (cited below as PAPER.md:<line>, section/e
 * readings of the paper where it is silent (R1..R16) are those listed in DESIGN.md section 3.
 * pins (tests/test_oracle_*.py, all run with -m "not gpu"): naive-DFT/closed-form checks of the
   discretisation, n=4 full-rank agreement with a brute-force 6D solver, second-order convergence to an
-  independent Strang solver, exact free streaming of the K-flow, Landau damping rate.
+  independent Strang solver, exact free streaming of the K-flow, Landau damping rate; step_bug (the unconventional
+  integrator the paper names): full-rank agreement with a brute-force forward RK4 step, first-order
+  convergence to the limit of Algorithm 2, robustness to a rank-deficient S (tests/test_oracle_bug.py).
   Parity unpinned: the choice among equally valid second-order variants (R8 which exponential RK,
   R10 order of directions) is pinned only up to "the brute-force solver that uses the same choice
   agrees, and the scheme converges at order 2"; results at rank r < 7 depend on the random padding.
@@ -385,6 +387,54 @@ def step_alg2(X, S, V, tau, gx, gv, e_scale=1.0, stats=None):
     X3, S7 = qr_mgs2(K4, gx.w, stats)                      # line 14
     return X3, S7, V1
 
+# --------------------------------------------------------------------------------------
+# The unconventional ("BUG") integrator
+# --------------------------------------------------------------------------------------
+def S_flow_forward(S, t, C1, C2, D1, D2):
+    """Galerkin S step of the unconventional integrator: the S equation is integrated FORWARD in time,
+    dS/dt = X^T F(X S V^T) V = -(sum_i D2_i S C1_i^T - sum_i D1_i S C2_i^T)  (eq. (10), is the same
+    right-hand side with the sign of the backward sub-flow (4)); one classical RK4 step (R11)."""
+    def rhs(Sm):
+        out = np.zeros_like(Sm)
+        for d in range(3):
+            out -= D2[d] @ Sm @ C1[d].T - D1[d] @ Sm @ C2[d].T
+        return out
+    k1 = rhs(S)
+    k2 = rhs(S + 0.5 * t * k1)
+    k3 = rhs(S + 0.5 * t * k2)
+    k4 = rhs(S + t * k3)
+    return S + (t / 6.0) * (k1 + 2.0 * k2 + 2.0 * k3 + k4)
+
+
+def step_bug(X, S, V, tau, gx, gv, e_scale=1.0, stats=None):
+    """One step of the unconventional (basis update & Galerkin) integrator, the paper's reference [4] (Ceruti &
+    Lubich), which the paper names as supported by its framework but does not write out (PAPER.md:29, 288);
+    restated here with the paper's sub-steps.  From (X0, S0, V0):
+      K step: K(t0) = X0 S0, eq. (9) with the coefficients of V0 over tau -> QR -> X1 (R discarded), M = <X1, X0>;
+      L step: L(t0) = V0 S0^T, eq. (11) with the coefficients of X0 over tau -> QR -> V1, N = <V1, V0>
+              (both start from the SAME initial data: they are independent, unlike in Algorithm 1);
+      S step: S(t0) = M S0 N^T, integrated forward with the coefficients of the NEW bases X1, V1 (S_flow_forward).
+    Readings (the paper is silent, R19): first order, so E is frozen at E0 of eq. (12) for all three sub-steps
+    (as Algorithm 1 does), the K and L flows are the Lie / exponential-Euler flows of Algorithm 1 (R13),
+    <.,.> are the h^3-weighted inner products of Fig. 2.
+    Returns (X1, S1, V1)."""
+    C1, C2, rho_t = coeff_C(V, gv)
+    K0 = X @ S
+    E0 = field(K0, rho_t, gx, e_scale)                     # eq. (12)
+    K1 = K_flow(K0, tau, C1, C2, E0, gx, 1)
+    X1, _ = qr_mgs2(K1, gx.w, stats)
+    M = gx.w * (X1.T @ X)
+    D1, D2 = coeff_D(X, E0, gx)                            # coefficients of the OLD basis X0
+    L0 = V @ S.T
+    L1 = L_flow(L0, tau, D1, D2, gv, 1)
+    V1, _ = qr_mgs2(L1, gv.w, stats)
+    N = gv.w * (V1.T @ V)
+    St = M @ S @ N.T
+    C1n, C2n, _ = coeff_C(V1, gv)
+    D1n, D2n = coeff_D(X1, E0, gx)
+    S1 = S_flow_forward(St, tau, C1n, C2n, D1n, D2n)
+    return X1, S1, V1
+
 
 # --------------------------------------------------------------------------------------
 # diagnostics (the quantities plotted in Figs. 4-7, PAPER.md:472, 609-621; definitions: R14)
@@ -415,6 +465,8 @@ def run(X, S, V, tau, nsteps, gx, gv, order=2, e_scale=1.0, probes=None):
     for _ in range(nsteps):
         if order == 2:
             X, S, V = step_alg2(X, S, V, tau, gx, gv, e_scale, stats)
+        elif order == "bug":
+            X, S, V = step_bug(X, S, V, tau, gx, gv, e_scale, stats)
         else:
             X, S, V = step_alg1(X, S, V, tau, gx, gv, e_scale, stats)
         hist.append(moments(X, S, V, gx, gv, e_scale))
