@@ -174,6 +174,9 @@ def main():
     ap.add_argument("--rank", type=int, default=0, help="override the rank of --config")
     ap.add_argument("--cpu-steps", type=int, default=1, help="oracle steps timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--unconventional", action="store_true",
+                    help="time the unconventional integrator (DLR_FLAG_UNCONVENTIONAL, first order) instead of Algorithm 2; "
+                         "not the headline metric: use with --no-cpu-baseline")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -190,6 +193,8 @@ def main():
     cfg = inputs.make_config(args.config, **over)
     workload = (f"BASELINE.json configs[{args.config - 1}]: {cfg['problem']} {cfg['n_x']}^3x{cfg['n_v']}^3, r={cfg['r']}, "
                 f"tau={cfg['tau']}, Algorithm 2")
+    if args.unconventional:
+        workload = workload.replace("Algorithm 2", "unconventional integrator (reference [4] of the paper)")
     config = {"workload": workload, "n": cfg["n"], "rank": cfg["r"], "tau": cfg["tau"], "parallelism": f"replicas x{args.gpus}",
               "l2": (f"working set {6 * 8 * max(cfg['n_x'], cfg['n_v']) ** 3 * cfg['r'] / 1e9:.2f} GB of factors and work buffers; "
                      "126 MB L2: no explicit flush, but at 64^3 a single 21 MB factor is L2-resident between consecutive passes "
@@ -228,7 +233,12 @@ def main():
 
     X, S, V = inputs.initial_factors(replicas.replica_cfg(cfg, rank))
     stream = torch.cuda.Stream(device=dev)
-    ctx = dlr.Dlr(dlr.config_from_inputs(cfg), device=dev, stream=stream)
+    if args.unconventional:
+        METRIC = METRIC.replace("2nd-order DLR step", "unconventional-integrator step (first order)")
+        X, S, V = inputs.weighted_start(replicas.replica_cfg(cfg, rank))
+    dcfg = (dlr.config_from_inputs(cfg, order=1, flags=dlr.FLAG_UNCONVENTIONAL) if args.unconventional
+            else dlr.config_from_inputs(cfg))
+    ctx = dlr.Dlr(dcfg, device=dev, stream=stream)
     Xd, Sd, Vd = (torch.from_numpy(np.ascontiguousarray(a.T)).to(dev) for a in (X, S, V))   # column-major on device
     tau = cfg["tau"]
 

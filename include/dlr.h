@@ -43,6 +43,12 @@ enum {
  * (DESIGN.md row a7'). With this flag the Lie L-flow of Algorithm 1 line 9 is run literally and its
  * column sums are used: same numbers up to rounding, one more pass family per step. For A/B tests. */
 #define DLR_FLAG_PREDICTOR_L_FLOW 1u
+/* dlr_step advances with the unconventional ("basis update & Galerkin") integrator, the paper's reference [4], which
+ * PAPER.md:29 and PAPER.md:288 name as supported by the framework without writing it out; here as oracle.step_bug
+ * restates it (reading R19): K step and L step BOTH from (X0, S0, V0) with E frozen at E0 of eq. (12) ->
+ * QR -> X1, V1;  M = <X1, X0>, N = <V1, V0> (h^3-weighted);  S step forward in time from M S0 N^T with the coefficients
+ * of X1, V1.  First order; requires order = 1; robust to a rank-deficient S0. */
+#define DLR_FLAG_UNCONVENTIONAL 2u
 
 /* Grid descriptors of Fig. 2: number of points, left extreme, right extreme of the
  * periodic box per direction (grid spacing h = (hi-lo)/n, points lo + i*h, i = 0..n-1).
@@ -54,7 +60,7 @@ typedef struct dlr_config {
     int32_t rank;
     int32_t order;      /* 2 = Algorithm 2; 1 = Algorithm 1 */
     double e_scale;     /* multiplies the electric field; 1.0 = the paper's equations, 0.0 = test hook "E = 0" */
-    uint32_t flags;     /* 0, or DLR_FLAG_PREDICTOR_L_FLOW */
+    uint32_t flags;     /* 0, DLR_FLAG_PREDICTOR_L_FLOW (order 2) or DLR_FLAG_UNCONVENTIONAL (order 1) */
 } dlr_config;
 
 /* Diagnostics the paper plots (Figs. 4-7). */

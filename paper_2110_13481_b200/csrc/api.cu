@@ -51,6 +51,7 @@ struct FlowTab {
     FlowTabPtrs p;
 };
 
+#define DLR_CROSS_CTAS 148
 struct Sub2Cfg { int L, groups, wpu, ctas; };      // launch shape of the direction-2 sub-flow (pass_sub2.cuh)
 struct ApplyCfg { int C, S, ctas; };              // chunk length, stages and grid of the A*Mat pass (pass_apply.cuh)
 struct Sub1Cfg { int use, NL, groups, wpu, ctas; };  // launch shape of the direction-1 sub-flow (pass_sub1.cuh); use = 0: CTA-tile kernel
@@ -92,6 +93,7 @@ struct dlr_ctx {
     double *gramF, *pgramF[3], *colsumF;     // and their totals (one row each): what the consumers read
     unsigned* grp_cnt;                       // 3 x DLR_CNT_STRIDE group counters, zero between kernels
     // small buffers
+    double *crossM, *crossN;      // per-CTA partial blocks of <X1, X0>, <V1, V0> (unconventional integrator)
     double *C1, *C2, *D1, *D2, *rho_t, *TC, *lamC, *TD, *lamD, *apply, *Rtot, *zsum, *mx, *mv, *mxp, *mvp, *mres, *esum;
     int* status;
     long long *pix, *piv;
@@ -218,7 +220,8 @@ int check_cfg(const dlr_config* c) {
     if (!is_pow2(nx) || !is_pow2(nv) || nx < 8 || nv < 8 || nx > 256 || nv > 256) return DLR_ERR_UNSUPPORTED;
     if (!dlr_rank_ops(c->rank)) return DLR_ERR_UNSUPPORTED;
     if (c->order != 1 && c->order != 2) return DLR_ERR_INVALID;
-    if ((c->flags & ~(uint32_t)DLR_FLAG_PREDICTOR_L_FLOW) != 0) return DLR_ERR_INVALID;
+    if ((c->flags & ~(uint32_t)(DLR_FLAG_PREDICTOR_L_FLOW | DLR_FLAG_UNCONVENTIONAL)) != 0) return DLR_ERR_INVALID;
+    if ((c->flags & DLR_FLAG_UNCONVENTIONAL) && c->order != 1) return DLR_ERR_INVALID;
     for (int d = 0; d < 3; d++) {
         if (!(c->x_hi[d] > c->x_lo[d]) || !(c->v_hi[d] > c->v_lo[d])) return DLR_ERR_INVALID;
         if (c->x_lo[d] != c->x_lo[0] || c->x_hi[d] != c->x_hi[0] || c->v_lo[d] != c->v_lo[0] || c->v_hi[d] != c->v_hi[0])
@@ -285,6 +288,7 @@ size_t carve(dlr_ctx* c, char* base) {
     c->TC = cv.take<double>(3 * RR); c->lamC = cv.take<double>(3 * R);
     c->TD = cv.take<double>(3 * RR); c->lamD = cv.take<double>(3 * R);
     c->apply = cv.take<double>(RR); c->Rtot = cv.take<double>(RR);
+    c->crossM = cv.take<double>((size_t)DLR_CROSS_CTAS * RR); c->crossN = cv.take<double>((size_t)DLR_CROSS_CTAS * RR);
     c->zsum = cv.take<double>(R);
     c->mx = cv.take<double>(5 * R); c->mv = cv.take<double>(5 * R); c->mres = cv.take<double>(8);
     c->mxp = cv.take<double>((size_t)5 * R * DLR_MCH); c->mvp = cv.take<double>((size_t)5 * R * DLR_MCH); c->esum = cv.take<double>(DLR_ECH);
@@ -576,7 +580,7 @@ void lpred_sums(dlr_ctx* c, double t3) {
 
 // The r x r work between two streaming phases, one launch (see k_post).
 struct PostM2 { const HostGrid* hg; double* M2; };
-struct PostS { double* S; double t; };
+struct PostS { double* S; double t; double sign; };      // sign: +1 eq. (10) as printed, -1 the forward Galerkin S step
 struct PostTab { const HostGrid* hg; const double *T, *lam, *Sin; int transS; double sgn, tsub, t3; const double* M2c; double nlsign; };
 void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
     PostArgs a;
@@ -587,7 +591,8 @@ void post(dlr_ctx* c, const PostM2* m2, const PostS* sf, const PostTab* tb) {
         for (int d = 0; d < 3; d++) a.pgram[d] = c->pgramF[d];             // the totals of the three coefficient passes
         a.m2scale = m2->hg->g.h3 / (double)m2->hg->g.n; a.M2 = m2->M2;     // 1D Parseval: sum_x u dv = (1/n) sum_k ...
     }
-    if (sf) { a.do_s = 1; a.S = sf->S; a.ts = sf->t; a.C1 = c->C1; a.C2 = c->C2; a.D1 = c->D1; a.D2 = c->D2; }
+    a.ssign = 1.0;
+    if (sf) { a.do_s = 1; a.S = sf->S; a.ts = sf->t; a.ssign = sf->sign; a.C1 = c->C1; a.C2 = c->C2; a.D1 = c->D1; a.D2 = c->D2; }
     if (tb) {
         a.do_tab = 1; a.Tm = tb->T; a.lam = tb->lam; a.Sin = tb->Sin; a.transS = tb->transS; a.g = tb->hg->g;
         a.sgn = tb->sgn; a.tsub = tb->tsub; a.t3 = tb->t3; a.M2c = tb->M2c; a.nlsign = tb->nlsign; a.o = c->ft.p;
@@ -715,8 +720,71 @@ void flow(dlr_ctx* c, const HostGrid& hg, const double* src, bool is_L, int orde
     CK(run_sub1(c, hg, a));                                      // sub-flow 1, second half, + Gram of the result
 }
 
+// One step of the unconventional integrator (DLR_FLAG_UNCONVENTIONAL; oracle.step_bug, the paper's reference [4] named in
+// PAPER.md:29, 288).  Reuses the Lie flows, the QR and the coefficient passes of Algorithm 1; new: the cross-Gram passes
+// M = <X1, X0>, N = <V1, V0> and the forward S step.  X1 goes to c->X1, V1 to c->W, and both are copied over X, V once
+// the old bases are no longer needed.
+void issue_step_bug(dlr_ctx* c, double tau) {
+    const HostGrid &gx = c->gx, &gv = c->gv;
+    const int R = c->R;
+    phase_mark(c, "start");
+    c->bytes_acc = 0.0;
+    if (!c->vh_valid) {
+        coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
+        const PostM2 m2C{&gv, c->C2};
+        post(c, &m2C, nullptr, nullptr);
+    }
+    phase_mark(c, "C coefficients (V0)");
+    field_fork(c, c->X, c->S, c->rho_t, 1, -1.0);                  // E0, eq. (12)
+    // K step from (X0, S0) -> X1 (the triangular factor is not used)
+    {
+        const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, tau, tau, c->C2, 1.0};
+        post(c, nullptr, nullptr, &tb);
+    }
+    flow(c, gx, c->X, false, 1, false);
+    qr(c, gx, c->X1, c->Sp, 0);
+    phase_mark(c, "K step + QR");
+    const int cx = (int)std::min<long long>(DLR_CROSS_CTAS, gx.g.N / 1024), cv = (int)std::min<long long>(DLR_CROSS_CTAS, gv.g.N / 1024);
+    const int ncx = std::max(1, cx), ncv = std::max(1, cv);
+    CK(c->ops->cross(c->X1, c->X, gx.g.N, c->crossM, ncx, c->st));
+    c->bytes_acc += 2.0 * fac_bytes(c, gx);
+    // L step from (V0, S0) with the coefficients of the OLD basis X0 -> V1
+    coeffs(c, gx, c->X, 2, c->D1, nullptr, c->TD, c->lamD);
+    {
+        const PostM2 m2D{&gx, c->D2};
+        const PostTab tb{&gv, c->TD, c->lamD, c->S, 1, +1.0, tau, tau, c->D2, -1.0};
+        post(c, &m2D, nullptr, &tb);
+    }
+    flow(c, gv, c->V, true, 1, false);
+    qr(c, gv, c->W, c->Sp, 1);
+    phase_mark(c, "L step + QR");
+    CK(c->ops->cross(c->W, c->V, gv.g.N, c->crossN, ncv, c->st));
+    c->bytes_acc += 2.0 * fac_bytes(c, gv);
+    CK(c->ops->bug_s0(c->crossM, ncx, c->crossN, ncv, gx.g.h3, gv.g.h3, c->S, c->st));     // S~ = M S0 N^T
+    // the new bases replace the old ones
+    CK(cudaMemcpyAsync(c->X, c->X1, (size_t)gx.g.N * R * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(c->V, c->W, (size_t)gv.g.N * R * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+    c->bytes_acc += 2.0 * fac_bytes(c, gx) + 2.0 * fac_bytes(c, gv);
+    // Galerkin S step forward in time with the coefficients of X1, V1 (E0 still in c->E)
+    coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
+    {
+        const PostM2 m2C{&gv, c->C2};
+        post(c, &m2C, nullptr, nullptr);
+    }
+    coeffs(c, gx, c->X, 2, c->D1, nullptr, c->TD, c->lamD);
+    {
+        const PostM2 m2D{&gx, c->D2};
+        const PostS sf{c->S, tau, -1.0};
+        post(c, &m2D, &sf, nullptr);
+    }
+    phase_mark(c, "S step (Galerkin)");
+    c->vh_valid = true;                                   // C(V1) are the next step's coefficients
+    c->bytes_step = c->bytes_acc;
+}
+
 // one step, issued on c->st (directly or under stream capture)
 void issue_step(dlr_ctx* c, double tau) {
+    if (c->cfg.flags & DLR_FLAG_UNCONVENTIONAL) { issue_step_bug(c, tau); return; }
     const int order = c->cfg.order;
     const double tp = order == 2 ? 0.5 * tau : tau;     // step size of the Algorithm-1 part
     const HostGrid &gx = c->gx, &gv = c->gv;
@@ -750,7 +818,7 @@ void issue_step(dlr_ctx* c, double tau) {
     coeffs(c, gx, Xp, 2, c->D1, nullptr, c->TD, c->lamD);
     phase_mark(c, "D coefficients (predictor)");
     {
-        const PostS sf{Sp, tp};
+        const PostS sf{Sp, tp, 1.0};
         const PostTab tb{&gv, c->TD, c->lamD, Sp, 1, +1.0, tp, tp, c->D2, -1.0};
         post(c, &m2D, &sf, &tb);
     }
@@ -785,7 +853,7 @@ void issue_step(dlr_ctx* c, double tau) {
     coeffs(c, gx, c->X, 2, c->D1, nullptr, c->TD, c->lamD);
     phase_mark(c, "D coefficients");
     {
-        const PostS sf{c->S, 0.5 * tau};
+        const PostS sf{c->S, 0.5 * tau, 1.0};
         const PostTab tb{&gv, c->TD, c->lamD, c->S, 1, +1.0, 0.5 * tau, tau, c->D2, -1.0};
         post(c, &m2D, &sf, &tb);
     }
@@ -801,7 +869,7 @@ void issue_step(dlr_ctx* c, double tau) {
     coeffs(c, gv, c->V, 1, c->C1, c->rho_t, c->TC, c->lamC);
     phase_mark(c, "C coefficients");
     {
-        const PostS sf{c->S, 0.5 * tau};
+        const PostS sf{c->S, 0.5 * tau, 1.0};
         const PostTab tb{&gx, c->TC, c->lamC, c->S, 0, -1.0, 0.25 * tau, 0.5 * tau, c->C2, 1.0};
         post(c, &m2C, &sf, &tb);
     }

@@ -19,6 +19,8 @@ struct PostArgs {
     int R, do_m2, do_s, do_tab;
     const double* pgram[3]; double m2scale; double* M2;
     double* S; double ts; const double *C1, *C2, *D1, *D2;
+    double ssign;           // +1: eq. (10) as printed (the backward sub-flow of the projector splitting); -1: the forward Galerkin
+                            // S step of the unconventional integrator (oracle.S_flow_forward)
     const double *Tm, *lam, *Sin; int transS; GridDev g; double sgn, tsub, t3; const double* M2c; double nlsign;
     FlowTabPtrs o;
 };
@@ -103,7 +105,7 @@ __global__ void __launch_bounds__(DLR_POST_THREADS) k_post(const PostArgs a) {
                         r1 = fma(-D1[1 * RR + aa * R + k], Qm[1 * RR + k * R + b], r1);
                         r2 = fma(-D1[2 * RR + aa * R + k], Qm[2 * RR + k * R + b], r2);
                     }
-                    rhs = (r0 + r1) + r2;
+                    rhs = a.ssign * ((r0 + r1) + r2);
                     kacc = fma(cw[stage], rhs, kacc);
                     Y[tid] = stage < 3 ? fma(cs[stage] * t, rhs, Sc[tid]) : fma(t / 6.0, kacc, Sc[tid]);
                 }

@@ -67,6 +67,8 @@ extern "C" const RankOps* CAT(dlr_rank_ops_, DLR_RANK)() {
         launch_sub1<R>,
         sub1_occupancy<R>,
         {launch_apply<R, true>, launch_apply<R, false>},
+        launch_cross<R>,
+        launch_bug_s0<R>,
         launch_post<R>,
         launch_lpred<R>,
         launch_chol_test};

@@ -8,6 +8,7 @@
 #include "post.cuh"
 #include "pass_sub1.cuh"
 #include "pass_apply.cuh"
+#include "pass_cross.cuh"
 
 // row-tile kernels without a transform (CholeskyQR passes, density, initial-state check)
 enum {
@@ -40,6 +41,8 @@ struct RankOps {
     cudaError_t (*sub1)(const Sub1Args&, int groups, int ctas, cudaStream_t);     // sub-flow 1, warp-autonomous (pass_sub1.cuh)
     int (*sub1_occ)(int log2n, int threads, size_t smem);                        // its resident CTAs per SM
     cudaError_t (*apply[2])(const ApplyArgs&, int ctas, cudaStream_t);          // A*Mat pass of CholeskyQR (pass_apply.cuh): [0] with Gram, [1] without
+    cudaError_t (*cross)(const double* A, const double* B, long long N, double* partial, int ctas, cudaStream_t);   // pass_cross.cuh
+    cudaError_t (*bug_s0)(const double* pm, int nm, const double* pn, int nn, double hx3, double hv3, double* S, cudaStream_t);
     cudaError_t (*post)(const PostArgs&, cudaStream_t);           // r x r work between two streaming phases (post.cuh)
     cudaError_t (*lpred)(const LpredArgs&, cudaStream_t);         // column sums of the predictor's L1 (post.cuh)
     cudaError_t (*chol_test)(const CholArgs&, double* mat_out, cudaStream_t);     // one CholeskyQR stage on its own (test hook)

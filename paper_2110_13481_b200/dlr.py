@@ -78,6 +78,7 @@ class DlrError(RuntimeError):
 
 
 FLAG_PREDICTOR_L_FLOW = 1
+FLAG_UNCONVENTIONAL = 2
 
 
 def make_config(n_x, n_v, x_lo, x_hi, v_lo, v_hi, rank, order=2, e_scale=1.0, flags=0):

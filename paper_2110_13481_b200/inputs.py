@@ -149,3 +149,24 @@ def probe_indices(cfg, nprobe=64, seed=7):
     ix = rng.integers(0, cfg["n_x"] ** 3, size=nprobe).astype(np.int64)
     iv = rng.integers(0, cfg["n_v"] ** 3, size=nprobe).astype(np.int64)
     return ix, iv
+
+
+def weighted_start(cfg, decay=1e-2, seed=77):
+    """(X0, S0, V0) of initial_factors(cfg) with a FULL-RANK coupling matrix: S0 = U diag(s) W^T, s from sigma_1 down to
+    decay * sigma_1 (geometric), U, W seeded orthogonal matrices that leave the physical first column alone.  Every basis
+    direction then carries weight, so the bases an integrator computes from K = X S, L = V S^T are determined to rounding
+    (needed where the result depends on them, e.g. the unconventional integrator: tests/test_gpu_parity.py)."""
+    X, S, V = initial_factors(cfg)
+    r = cfg["r"]
+    rng = np.random.default_rng(seed)
+    mats = []
+    for _ in range(2):
+        A = rng.standard_normal((r, r))
+        A[0, :] = 0.0
+        A[:, 0] = 0.0
+        A[0, 0] = 1.0
+        Q, _ = np.linalg.qr(A)
+        mats.append(Q)
+    s = S[0, 0] * np.logspace(0.0, np.log10(decay), r)
+    return X, mats[0] @ np.diag(s) @ mats[1].T, V
+

@@ -77,3 +77,16 @@ def test_bug_step_structure_and_rank_deficient_start():
     # tau -> 0: the step tends to the identity on f
     X2, S2, V2 = O.step_bug(X, S, V, 1e-6, gx, gv)
     assert np.abs(X2 @ S2 @ V2.T - X @ S @ V.T).max() < 1e-5 * np.abs(X @ S @ V.T).max()
+
+
+def test_weighted_start_is_full_rank_and_keeps_the_bases():
+    """inputs.weighted_start (the well-posed start of the GPU parity test): same orthonormal X0, V0, S0 with singular
+    values sigma_1 ... decay * sigma_1, first row/column untouched by the seeded rotations"""
+    cfg = inputs.make_config(1, n=8, r=10)
+    gx, gv = grids(cfg)
+    X0, S0, V0 = inputs.initial_factors(cfg)
+    X, S, V = inputs.weighted_start(cfg, decay=1e-2)
+    assert np.array_equal(X, X0) and np.array_equal(V, V0)
+    sv = np.linalg.svd(S, compute_uv=False)
+    assert np.allclose(sv, S0[0, 0] * np.logspace(0, -2, 10), rtol=1e-12)
+    assert abs(S[0, 0] - S0[0, 0]) < 1e-12 * S0[0, 0] and np.abs(S[0, 1:]).max() < 1e-14 and np.abs(S[1:, 0]).max() < 1e-14
