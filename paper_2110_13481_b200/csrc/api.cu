@@ -503,7 +503,7 @@ void setup_sub1(dlr_ctx* c, const HostGrid& hg, Sub1Cfg& sc) {
     const size_t unit = sub1_unit_elems(n, R, sc.NL) * 16;
     sc.wpu = unit <= 24 * 1024 ? 1 : 2;
     { const int w = tune("s1u", 0); if (w == 1 || w == 2 || w == 4) sc.wpu = w; }
-    sc.use = unit <= 48 * 1024 && tune("s1", 1) != 0;
+    sc.use = unit <= (size_t)tune("s1max", 48) * 1024 && tune("s1", 1) != 0;
     sc.groups = 8 / sc.wpu;
     { const int w = tune("s1w", 0); if (w >= 1 && w <= 8 / sc.wpu) sc.groups = w; }
     const size_t target = (size_t)tune("s1sm", 110) * 1024;

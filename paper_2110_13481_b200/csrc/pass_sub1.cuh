@@ -135,6 +135,7 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
 #pragma unroll
                     for (int J = I; J < NB; J++) dmma884(gacc[GramShape<R>::tp(I, J)], frag[I], frag[J]);
             }
+            gp.sync();      // every warp of the group has read the unit before the inverse transform rewrites it (two-warp units!)
         }
         if constexpr (p.ng >= 2) {
             wf_group<p.g[p.ng - 1], true>(z, zl, R, lg, 0, p.g[p.ng - 1], tab, gp);

@@ -338,3 +338,25 @@ def test_nothing_is_written_outside_the_workspace(n_x, n_v, r, order):
     assert np.isfinite(f).all() and m["nonfinite"] == 0
     assert ctx.check_guards()
     ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,r,reps", [(32, 20, 40), (64, 15, 12)])
+def test_units_owned_by_two_warps_are_bit_reproducible(n, r, reps):
+    """regression test of a race found in round 2: where a unit of the sub-flow-1 kernel exceeds 24 KB (here 25.6 KB and
+    34.5 KB) two warps own it, and one warp's Gram sweep of the unit must finish before the other starts the inverse
+    transform (pass_sub1.cuh).  Without the group barrier ~2.5 % of the runs differed in the last digits of the Gram
+    matrix (found by test_two_contexts_of_different_shape_in_one_process; compute-sanitizer is closed on this pool).
+    Many short runs of Algorithm 2 (whose Strang flows use that Gram path) must give bit-identical factors."""
+    import hashlib
+    from paper_2110_13481_b200 import dlr
+    cfg = inputs.make_config(1, n=n, r=r)
+    X, S, V = inputs.initial_factors(cfg)
+    seen = set()
+    for _ in range(reps):
+        ctx = dlr.Dlr(dlr.config_from_inputs(cfg))
+        ctx.set_initial(X, S, V)
+        ctx.run(cfg["tau"], 2)
+        seen.add(tuple(hashlib.md5(np.ascontiguousarray(a).tobytes()).hexdigest() for a in ctx.get_factors()))
+        ctx.close()
+    assert len(seen) == 1
