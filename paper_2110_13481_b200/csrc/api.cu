@@ -477,7 +477,7 @@ void setup_sub2(dlr_ctx* c, const HostGrid& hg, Sub2Cfg& sc) {
     const int n = hg.g.n, M = n / 2;
     sc.L = n <= 64 ? std::min(M, 8) : 4;
     sc.wpu = n >= 256 ? 2 : 1;
-    sc.groups = 4;
+    sc.groups = n >= 256 ? 2 : 4;                 // measured at 256^3, r = 20: 2123 -> 1956 us per pass with two 2-warp groups
     { const int l = tune("s2l", 0); if (is_pow2(l) && l <= M) sc.L = l; }
     { const int w = tune("s2w", 0); if (w >= 1 && w <= 8) sc.groups = w; }
     { const int w = tune("s2u", 0); if (w == 1 || w == 2 || w == 4) sc.wpu = w; }
@@ -506,7 +506,9 @@ void setup_sub1(dlr_ctx* c, const HostGrid& hg, Sub1Cfg& sc) {
     sc.use = unit <= (size_t)tune("s1max", 48) * 1024 && tune("s1", 1) != 0;
     sc.groups = 8 / sc.wpu;
     { const int w = tune("s1w", 0); if (w >= 1 && w <= 8 / sc.wpu) sc.groups = w; }
-    const size_t target = (size_t)tune("s1sm", 110) * 1024;
+    // up to rank 10 two CTAs share an SM (110 KB each); above, one CTA owns it (register budget): more units per CTA
+    // (128^3, r = 15: 365 -> 332 us per pass)
+    const size_t target = (size_t)tune("s1sm", R > 10 ? 200 : 110) * 1024;
     while (sc.groups > 1 && sub1_smem_bytes(n, R, sc.NL, sc.groups) > target) sc.groups--;
     if (sub1_smem_bytes(n, R, sc.NL, sc.groups) > SMEM_MAX - 1024) sc.use = 0;
     if (!sc.use) return;
@@ -641,14 +643,15 @@ void field_join(dlr_ctx* c) {
 }
 
 void setup_apply(dlr_ctx* c, const HostGrid& hg, ApplyCfg& ac) {
-    // A*Mat pass of the QR (pass_apply.cuh): chunks of 512 points while a stage (r columns) stays near 41 KB, else 256, and as
-    // many stages as fit into ~190 KB.  Measured at 64^3, r = 10: 512 x 4 stages 20.5 us per pass, 256 x 8 stages 22 us, 128: 35 us
-    // (per-chunk barrier and copy issue), against 21.5 us of the CTA-tile kernel it replaces
+    // A*Mat pass of the QR (pass_apply.cuh): chunks of 512 points (4 KB per column and bulk copy) and as many stages as fit
+    // into ~190 KB, at least two.  Measured: 64^3, r = 10: 512 x 4 stages 20.5 us per pass, 256 x 8: 22, 128 x 8: 35 (per-chunk
+    // barrier and copy issue), 1024 x 2: 21.5; HBM-resident shapes want the larger copies even with few stages:
+    // 128^3, r = 15: 512 x 3 stages 113 us against 167 for 256 x 6; 256^3, r = 20: 512 x 2 stages -20 % against 256 x 4
     const int R = c->R;
-    ac.C = ((size_t)R * apply_cs(512) * 8 <= 48 * 1024 && hg.g.N % 512 == 0) ? 512 : 256;
+    ac.C = hg.g.N % 512 == 0 ? 512 : 256;
     { const int v = tune("apc", 0); if (v >= 64 && v % 64 == 0 && hg.g.N % v == 0) ac.C = v; }
     const size_t stage = (size_t)R * apply_cs(ac.C) * 8;
-    ac.S = (int)std::min<size_t>(8, (190 * 1024) / stage);
+    ac.S = (int)std::max<size_t>(2, std::min<size_t>(8, (190 * 1024) / stage));
     { const int v = tune("aps", 0); if (v >= 2 && v <= 8) ac.S = v; }
     while (ac.S > 2 && apply_smem_bytes(R, ac.C, ac.S) > SMEM_MAX - 1024) ac.S--;
     ac.ctas = (int)std::min<long long>(c->nsm, hg.g.N / ac.C);
