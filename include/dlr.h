@@ -35,7 +35,8 @@ enum {
     DLR_ERR_WORKSPACE = -3,        /* workspace too small or misaligned */
     DLR_ERR_CUDA = -4,             /* a CUDA runtime call failed (see dlr_last_cuda_error) */
     DLR_ERR_NOT_ORTHONORMAL = -5,  /* dlr_set_initial: h^3 X^T X or h^3 V^T V differs from I by > 1e-10 */
-    DLR_ERR_NO_STATE = -6          /* dlr_step / dlr_moments before dlr_set_initial */
+    DLR_ERR_NO_STATE = -6,         /* dlr_step / dlr_moments before dlr_set_initial */
+    DLR_ERR_TOO_LARGE = -7         /* dlr_probe_noalloc: more probes than the static device scratch holds */
 };
 
 /* dlr_config.flags: the predictor of Algorithm 2 (line 1) needs of its L step only rho(L^1) = L^1^T omega_v
@@ -165,6 +166,26 @@ const char* dlr_last_cuda_error(dlr_ctx* ctx);
  * latched error and drops the state (it may be half-updated): dlr_set_initial must follow. A sticky CUDA error
  * (illegal address, ...) cannot be cleared: the next call fails again. */
 int dlr_clear_error(dlr_ctx* ctx);
+
+/* f at grid-index pairs WITHOUT any device allocation, context or workspace: f_probe[p] = X[probe_ix[p],:] S
+ * V[probe_iv[p],:]^T (rows of F = X S V^T), the same kernel arithmetic as the probes of dlr_moments.
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses that forbid it): the
+ * probe indices and results pass through a file-scope static device array of DLR_NOALLOC_MAX_PROBES * 24 bytes that every
+ * GPU loading the library holds until the process exits; the call makes no cudaMalloc/cudaFree.
+ *   d_X (N_x x rank), d_S (rank x rank), d_V (N_v x rank): DEVICE arrays in the layout at the top of this file (e.g.
+ *   the output of dlr_get_factors(..., on_device = 1)), owned by the caller, all on the device that owns d_X (which the
+ *   call makes current and restores); probe_ix, probe_iv, f_probe: HOST arrays of n_probe entries; cuda_stream: the
+ *   stream the work is issued on (0 = legacy default).  Synchronises that stream.
+ * Errors: n_probe > DLR_NOALLOC_MAX_PROBES -> DLR_ERR_TOO_LARGE (nothing is launched; split the call); null pointers,
+ * non-positive sizes, an index outside [0, N) or a non-device d_X -> DLR_ERR_INVALID; CUDA failures -> DLR_ERR_CUDA.
+ * dlr_noalloc_last_error() returns the message of the calling thread's last failed call ("" if none).
+ * ALL calls share the one array: calls that overlap on the GPU (different streams or host threads) race on it and must
+ * be serialised by the caller.  The array keeps the previous call's contents; nothing in it needs to start at zero
+ * (a call overwrites every slot it reads). */
+#define DLR_NOALLOC_MAX_PROBES 4096
+int dlr_probe_noalloc(const double* d_X, const double* d_S, const double* d_V, int64_t N_x, int64_t N_v, int rank,
+                      int n_probe, const int64_t* probe_ix, const int64_t* probe_iv, double* f_probe, void* cuda_stream);
+const char* dlr_noalloc_last_error(void);
 
 #ifdef __cplusplus
 }

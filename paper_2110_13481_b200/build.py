@@ -30,6 +30,7 @@ def build(force=False, verbose=False):
     for r in RANKS:
         jobs.append((os.path.join(CSRC, "rank_inst.cu"), os.path.join(OBJ, f"rank_{r}.o"), [f"-DDLR_RANK={r}"]))
     jobs.append((os.path.join(CSRC, "api.cu"), os.path.join(OBJ, "api.o"), []))
+    jobs.append((os.path.join(CSRC, "noalloc.cu"), os.path.join(OBJ, "noalloc.o"), []))
 
     def run(job):
         src, obj, extra = job

@@ -908,6 +908,7 @@ const char* dlr_strerror(int code) {
         case DLR_ERR_CUDA: return "CUDA error";
         case DLR_ERR_NOT_ORTHONORMAL: return "initial factors are not orthonormal";
         case DLR_ERR_NO_STATE: return "no state set";
+        case DLR_ERR_TOO_LARGE: return "size exceeds the static device scratch (DLR_NOALLOC_MAX_PROBES)";
         default: return "unknown error";
     }
 }

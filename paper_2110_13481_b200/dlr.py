@@ -14,7 +14,8 @@ LIB_PATH = os.path.join(_HERE, "libdlr_b200.so")
 
 DLR_OK = 0
 ERRORS = {0: "DLR_OK", -1: "DLR_ERR_INVALID", -2: "DLR_ERR_UNSUPPORTED", -3: "DLR_ERR_WORKSPACE", -4: "DLR_ERR_CUDA",
-          -5: "DLR_ERR_NOT_ORTHONORMAL", -6: "DLR_ERR_NO_STATE"}
+          -5: "DLR_ERR_NOT_ORTHONORMAL", -6: "DLR_ERR_NO_STATE", -7: "DLR_ERR_TOO_LARGE"}
+NOALLOC_MAX_PROBES = 4096
 
 
 class dlr_config(ctypes.Structure):
@@ -67,6 +68,9 @@ def lib():
         L.dlr_last_cuda_error.argtypes = [vp]
         L.dlr_last_cuda_error.restype = ctypes.c_char_p
         L.dlr_clear_error.argtypes = [vp]
+        L.dlr_probe_noalloc.argtypes = [vp, vp, vp, ctypes.c_int64, ctypes.c_int64, ip, ip, vp, vp, vp, vp]
+        L.dlr_noalloc_last_error.argtypes = []
+        L.dlr_noalloc_last_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -111,6 +115,23 @@ def _ptr(a):
     if isinstance(a, np.ndarray):
         return a.ctypes.data
     return a.data_ptr()
+
+
+def probe_noalloc(X, S, V, probe_ix, probe_iv, stream=None):
+    """dlr_probe_noalloc: f = X S V^T at index pairs, no device allocation (static device scratch, at most
+    NOALLOC_MAX_PROBES pairs per call).  X (r, N_x), S (r, r), V (r, N_v): CUDA tensors holding the ABI's column-major
+    layout (row c of the tensor = column c of the factor); probe_ix, probe_iv: host integer sequences -> numpy f"""
+    import torch
+    r = S.shape[0]
+    ix = np.ascontiguousarray(probe_ix, dtype=np.int64)
+    iv = np.ascontiguousarray(probe_iv, dtype=np.int64)
+    f = np.empty(len(ix), dtype=np.float64)
+    st = stream if stream is not None else torch.cuda.current_stream(X.device)
+    rc = lib().dlr_probe_noalloc(X.data_ptr(), S.data_ptr(), V.data_ptr(), X.numel() // r, V.numel() // r, r, len(ix),
+                                 _ptr(ix), _ptr(iv), _ptr(f), st.cuda_stream)
+    if rc != DLR_OK:
+        raise DlrError(rc, "dlr_probe_noalloc", lib().dlr_noalloc_last_error().decode())
+    return f
 
 
 class Dlr:
