@@ -33,6 +33,8 @@ const RankOps* dlr_rank_ops(int R) {
     }
 }
 
+thread_local int g_dlr_pdl = 0;     // common.cuh: dlr_launch sets the programmatic-serialisation attribute while this is 1
+
 namespace {
 
 struct HostGrid {
@@ -99,6 +101,7 @@ struct dlr_ctx {
     long long *pix, *piv;
     double* pf;
     int probe_cap;
+    int pdl;                      // programmatic dependent launch for the kernels of a step (see dlr_create)
     FlowTab ft;
     double* small_end;
     bool has_state, vh_valid, profiling;
@@ -117,6 +120,12 @@ struct dlr_ctx {
 namespace {
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// programmatic dependent launch (common.cuh) is on while dlr_step issues or captures a step, off in every other entry point
+struct PdlScope {
+    explicit PdlScope(int on) { g_dlr_pdl = on; }
+    ~PdlScope() { g_dlr_pdl = 0; }
+};
 
 // every entry point that touches the device runs with the context's device current and restores the caller's
 struct DevGuard {
@@ -294,6 +303,9 @@ size_t carve(dlr_ctx* c, char* base) {
     c->mxp = cv.take<double>((size_t)5 * R * DLR_MCH); c->mvp = cv.take<double>((size_t)5 * R * DLR_MCH); c->esum = cv.take<double>(DLR_ECH);
     c->status = cv.take<int>(4);
     c->probe_cap = 4096;
+    // Programmatic dependent launch pays where a pass is short (L2-resident factors: 64^3, r = 10: 1.029 -> 1.009 ms/step);
+    // with HBM-resident factors the early-resident CTAs of the next pass only take slots (128^3, r = 15: 11.43 -> 11.51 ms)
+    c->pdl = tune("pdl", 8.0 * (double)std::max(c->gx.g.N, c->gv.g.N) * c->R <= 64.0 * 1024 * 1024 ? 1 : 0);
     c->pix = cv.take<long long>(c->probe_cap); c->piv = cv.take<long long>(c->probe_cap); c->pf = cv.take<double>(c->probe_cap);
     const int nmax = std::max(c->gx.g.n, c->gv.g.n);
     c->ft.p.mats = cv.take<double>(8 * RR);
@@ -1068,6 +1080,7 @@ int dlr_step(dlr_ctx* c, double tau) {
     DevGuard guard(c->dev);
     if (!c->has_state) return DLR_ERR_NO_STATE;
     if (c->last_err != cudaSuccess) return DLR_ERR_CUDA;
+    PdlScope pdl(c->profiling ? 0 : c->pdl);      // profiling records events between the launches: plain launches
     if (c->profiling || !c->vh_valid) {
         // first step after set_initial (it also computes the C coefficients of V0) or profiling: direct launches
         for (auto& p : c->phases) cudaEventDestroy(p.ev);

@@ -40,6 +40,39 @@ inline cudaError_t dlr_optin_smem(K kern) {
     return e;
 }
 
+// ---------------------------------------------------------------- programmatic dependent launch
+// Every kernel of the step is launched with programmatic stream serialisation (dlr_launch): the next kernel of the stream
+// may become resident while this one drains, so its launch latency and whatever it does before pdl_wait() (twiddle
+// tables that dlr_create wrote: nothing a kernel of the step produces) overlap the tail of its predecessor.  pdl_wait()
+// returns once the preceding kernel of the stream has completed and its writes are visible; EVERY kernel calls it before
+// its first access to step data (also before overwriting what an earlier kernel reads), which keeps the chain transitive.
+// pdl_trigger() only moves the point at which the successor may become resident; correctness never depends on it.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() {
+#ifndef DLR_PDL_NO_TRIGGER
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+}
+
+// 16-byte asynchronous copy global -> shared (LDGSTS): a thread can have all the elements of its tile share in flight at once
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
+
+extern thread_local int g_dlr_pdl;      // set by the issuing entry point of api.cu for the duration of a call (0 = plain launches)
+
+template <class... KA, class... A>
+inline cudaError_t dlr_launch(void (*kern)(KA...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, A&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = g_dlr_pdl ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KA(args)...);
+}
+
 // ---------------------------------------------------------------- complex helpers
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }

@@ -64,6 +64,8 @@ __host__ inline size_t d1_smem_bytes(int n, int RMAX, int T, bool needE, int nma
 
 template <int RIN, int ROUT, int IN_MODE, int OP, int GRAM, int OUT_MODE>
 __global__ void __launch_bounds__(DLR_THREADS, ((RIN > ROUT ? RIN : ROUT) <= 16 ? 2 : 1)) k_d1(const D1Args a) {
+    pdl_wait();
+    pdl_trigger();
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
     constexpr int NMAT = OP == D1_OP_MATVEC ? RIN * ROUT : 0;
     const int n = a.g.n, M = n >> 1, lg = a.g.log2n, logM = lg - 1, T = a.T;
@@ -241,6 +243,5 @@ inline cudaError_t launch_d1(const D1Args& a, cudaStream_t st) {
     auto kern = k_d1<RIN, ROUT, IN_MODE, OP, GRAM, OUT_MODE>;
     const size_t sm = d1_smem_bytes(a.g.n, RMAX, a.T, false, (NMAT + 1) & ~1);
     const unsigned grid = (unsigned)(((long long)a.g.n * a.g.n) / a.T);
-    kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(kern, grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st, a);
 }

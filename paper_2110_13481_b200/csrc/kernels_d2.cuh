@@ -21,6 +21,8 @@ __host__ inline size_t d2_smem_bytes(int n, int T2, int NB) {
 
 template <bool INV>
 __global__ void __launch_bounds__(DLR_THREADS, 3) k_d2(const D2Args a) {
+    pdl_wait();
+    pdl_trigger();
     const int n = a.g.n, nh = a.g.nh, lg = a.g.log2n, T2 = a.T2, NB = a.NB;
     const int nlines = T2 * NB, LP = nlines | 1;
     extern __shared__ double2 smem2[];
@@ -70,6 +72,5 @@ inline cudaError_t launch_d2(const D2Args& a, cudaStream_t st) {
     const size_t sm = d2_smem_bytes(a.g.n, a.T2, a.NB);
     const long long nslab = (long long)a.ncols * a.g.n;
     const unsigned grid = (unsigned)(a.nchunks * ((nslab + a.NB - 1) / a.NB));
-    kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(kern, grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st, a);
 }

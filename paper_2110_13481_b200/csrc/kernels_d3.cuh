@@ -28,6 +28,8 @@ __host__ inline size_t d3_smem_bytes(int n, int RMAX, int T, int nmat) {
 
 template <int RIN, int ROUT, int FOP, bool UNUSED>
 __global__ void __launch_bounds__(DLR_THREADS, 2) k_d3(const D3Args a) {
+    pdl_wait();
+    pdl_trigger();
     constexpr int RMAX = RIN > ROUT ? RIN : ROUT;
     const int n = a.g.n, nh = a.g.nh, lg = a.g.log2n, T = a.T;
     const int lt = __ffs(T) - 1;                                 // T is a power of two
@@ -94,6 +96,5 @@ inline cudaError_t launch_d3(const D3Args& a, cudaStream_t st) {
     const size_t sm = d3_smem_bytes(a.g.n, RMAX, a.T, 0);
     const long long plane = (long long)a.g.nh * a.g.n;
     const unsigned grid = (unsigned)((plane + a.T - 1) / a.T);
-    kern<<<grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(kern, grid, a.threads > 0 ? a.threads : DLR_THREADS, sm, st, a);
 }

@@ -117,6 +117,15 @@ __device__ __forceinline__ void dir_weights(const DirGeom& gm, const double2* Et
     }
 }
 
+// The loop over output-column pairs of the streamed r x r products stays ROLLED: a thread runs these bodies once or twice
+// per tile, so unrolled code is fetched once per use (ncu: 17 % of the stall samples of the third sub-flow were
+// instruction-fetch stalls with 4100 instructions of straight-line code); x[] is indexed by the unrolled inner loop only.
+#ifdef DLR_CO_UNROLLED
+#define DLR_CO_LOOP _Pragma("unroll")
+#else
+#define DLR_CO_LOOP _Pragma("unroll 1")
+#endif
+
 // copy a dense [R][R] matrix into the padded layout (pads zeroed); all threads of the CTA
 template <int R>
 __device__ __forceinline__ void mat_stage(double* dst, const double* __restrict__ src) {
@@ -152,7 +161,7 @@ __device__ __forceinline__ void dir_matvec(double2 (&x)[R], const double* A) {  
 template <int R>
 __device__ __forceinline__ void dir_matvec_store(const double2 (&x)[R], const double* A, double2* out, int stride) {
     constexpr int RS = mat_rs(R);
-#pragma unroll
+DLR_CO_LOOP
     for (int co = 0; co < R; co += 2) {
         double2 a0 = make_double2(0.0, 0.0), a1 = a0;
 #pragma unroll
@@ -172,7 +181,7 @@ template <int R>
 __device__ __forceinline__ void dir_nonlin(const double2 (&m)[R], double2* gout, int stride, const double* Q, double2 w0,
                                            double2 w1, double2 w2) {
     constexpr int RS = mat_rs(R), MS = mat_ms(R);
-#pragma unroll
+DLR_CO_LOOP
     for (int co = 0; co < R; co += 2) {
         double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0, t0 = s0, t1 = s0, t2 = s0;
 #pragma unroll
@@ -192,6 +201,32 @@ __device__ __forceinline__ void dir_nonlin(const double2 (&m)[R], double2* gout,
             gout[(co + 1) * stride] = make_double2(fma(w0.x, t0.x, fma(w1.x, t1.x, w2.x * t2.x)),
                                                    fma(w0.y, t0.y, fma(w1.y, t1.y, w2.y * t2.y)));
     }
+}
+
+// Real-space phase of the exponential Runge-Kutta stages:
+//   x = scale * src [* Min, written back to src];  dst = N'(x) = sum_i w_i o (x Q_i)          (src, dst: column 0 of (e, l))
+// (measured at 64^3, r = 10: inlined 72.3 us per ETD2RK launch, as one shared non-inlined copy 75.1: the call passes
+// its arguments through the stack)
+template <int R, int DIR, int DW>
+__device__ __forceinline__ void etd_realspace(double2* z, int LPZ, int pitems, int src_off, int dst_off, double scale,
+                                           const double* min_, const double* Q, const DirGeom gm, const double2* Et) {
+    const int L = gm.L, lL = gm.lL;
+    for (int w = threadIdx.x; w < pitems; w += blockDim.x) {
+        const int l = w & (L - 1), e = w >> lL;
+        double2* p = z + (size_t)e * LPZ + l;
+        double2 x[R];
+#pragma unroll
+        for (int c = 0; c < R; c++) { x[c] = p[src_off + c * L]; x[c].x *= scale; x[c].y *= scale; }
+        if (min_ != nullptr) {
+            dir_matvec_store<R>(x, min_, p + src_off, L);
+#pragma unroll
+            for (int c = 0; c < R; c++) x[c] = p[src_off + c * L];       // this thread's own stores
+        }
+        double2 w0, w1, w2;
+        dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
+        dir_nonlin<R>(x, p + dst_off, L, Q, w0, w1, w2);                 // x is fully in registers: dst may be src
+    }
+    __syncthreads();
 }
 
 // emit functions for mma_tiles_reduce: accumulator index a and tile position pos -> entry of the partial row
@@ -234,9 +269,7 @@ k_dir(const DirArgs a) {
         gm.ia = (int)blockIdx.x >> ltp;
         gm.j0 = ((int)blockIdx.x & ((1 << ltp) - 1)) << lL;
     }
-    if (MIX && a.min_ != nullptr) mat_stage<R>(mats, a.min_);
-    if (MIX && a.mout != nullptr) mat_stage<R>(mats + MS, a.mout);
-    if (ETD) { mat_stage<R>(mats + 2 * MS, a.Q); mat_stage<R>(mats + 3 * MS, a.Q + R * R); mat_stage<R>(mats + 4 * MS, a.Q + 2 * R * R); }
+    pdl_wait();
     const size_t N2 = (size_t)(a.g.N >> 1);
     const double invn = 1.0 / (double)n;
 
@@ -268,7 +301,7 @@ k_dir(const DirArgs a) {
             const int items = nl << lg;
             for (int w = tid; w < items; w += nth) {
                 const int l = w & (L - 1), e = (w >> lL) & (n - 1), c = w >> (lL + lg);
-                z[(size_t)e * LPZ + c * L + l] = in2[(size_t)c * N2 + dir_index<DIR>(gm, e, l)];
+                cp_async16(z + (size_t)e * LPZ + c * L + l, in2 + (size_t)c * N2 + dir_index<DIR>(gm, e, l));
             }
         }
         if (DW == DW_E) {
@@ -288,13 +321,19 @@ k_dir(const DirArgs a) {
                     const int items = L << lg;
                     for (int w = tid; w < items; w += nth) {
                         const int l = w & (L - 1), e = w >> lL;
-                        Ed[e * L + l] = e2[dir_index<DIR>(gm, e, l)];
+                        cp_async16(Ed + e * L + l, e2 + dir_index<DIR>(gm, e, l));
                     }
                 }
             }
         }
     }
+    // the mixing matrices are staged while the asynchronous copies of the tile (directions 2, 3) are in flight
+    if (MIX && a.min_ != nullptr) mat_stage<R>(mats, a.min_);
+    if (MIX && a.mout != nullptr) mat_stage<R>(mats + MS, a.mout);
+    if (ETD) { mat_stage<R>(mats + 2 * MS, a.Q); mat_stage<R>(mats + 3 * MS, a.Q + R * R); mat_stage<R>(mats + 4 * MS, a.Q + 2 * R * R); }
+    cp_async_wait_all();
     __syncthreads();
+    pdl_trigger();                                            // one tile per CTA: every CTA of the grid has started by now
     const int pitems = n << lL;                               // tile points (e, l)
 
     if (DOP == DOP_COEFF) {
@@ -403,22 +442,8 @@ k_dir(const DirArgs a) {
     if (ETD) {
         // -------------------------------------------------------------- third sub-flow, exponential Runge-Kutta
         const double* Q = mats + 2 * MS;
-        for (int w = tid; w < pitems; w += nth) {             // m = A Min,  g0 = N'(m)
-            const int l = w & (L - 1), e = w >> lL;
-            double2* p = z + (size_t)e * LPZ + l;
-            double2 x[R];
-#pragma unroll
-            for (int c = 0; c < R; c++) x[c] = p[c * L];
-            if (a.min_ != nullptr) {
-                dir_matvec<R>(x, mats);
-#pragma unroll
-                for (int c = 0; c < R; c++) p[c * L] = x[c];
-            }
-            double2 w0, w1, w2;
-            dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
-            dir_nonlin<R>(x, p + nl, L, Q, w0, w1, w2);
-        }
-        __syncthreads();
+        // m = A Min,  g0 = N'(m)
+        etd_realspace<R, DIR, DW>(z, LPZ, pitems, 0, nl, 1.0, a.min_ != nullptr ? mats : nullptr, Q, gm, Et);
         // Fourier-space stages fused into the middle FFT group (fft_mid2): the spectra of m and g0 never make a round
         // trip through shared memory.  a = e^z M^ + t phi1 G0^  (stage-1 state);  ETD2RK keeps  e^z M^ + t (phi1 - phi2) G0^
         // in buffer A (spectral) and adds t phi2 G1^ to it after the second evaluation of the real-space term.
@@ -438,17 +463,7 @@ k_dir(const DirArgs a) {
                 bv = ah;                                      // inverse-transformed for N'(a)
             });
             fft_lines_c<true>(z + nl, LPZ, nl, lg, true);
-            for (int w = tid; w < pitems; w += nth) {         // g1 = N'(a)
-                const int l = w & (L - 1), e = w >> lL;
-                double2* p = z + (size_t)e * LPZ + nl + l;
-                double2 x[R];
-#pragma unroll
-                for (int c = 0; c < R; c++) { x[c] = p[c * L]; x[c].x *= invn; x[c].y *= invn; }
-                double2 w0, w1, w2;
-                dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
-                dir_nonlin<R>(x, p, L, Q, w0, w1, w2);            // x is fully in registers: in-place is safe
-            }
-            __syncthreads();
+            etd_realspace<R, DIR, DW>(z, LPZ, pitems, nl, nl, invn, nullptr, Q, gm, Et);      // g1 = N'(a), in place
             fft_lines_c<false>(z + nl, LPZ, nl, lg, true);
             fft_mid2<false, true, true, false, true, false>(z, nl, LPZ, nl, lg, [&](double2& av, double2& bv, int e, int line) {
                 av = cadd(av, cmul(bv, __ldg(a.f2b + (size_t)e * R + (line >> lL))));
@@ -461,9 +476,11 @@ k_dir(const DirArgs a) {
             double2 x[R];
 #pragma unroll
             for (int c = 0; c < R; c++) { x[c] = p[c * L]; x[c].x *= invn; x[c].y *= invn; }
-            if (a.mout != nullptr) dir_matvec<R>(x, mats + MS);
+            if (a.mout != nullptr) dir_matvec_store<R>(x, mats + MS, p, L);
+            else {
 #pragma unroll
-            for (int c = 0; c < R; c++) p[c * L] = x[c];
+                for (int c = 0; c < R; c++) p[c * L] = x[c];
+            }
         }
         __syncthreads();
     }
@@ -530,6 +547,5 @@ inline cudaError_t launch_dir(const DirArgs& a, cudaStream_t st) {
     constexpr bool ETD = (DOP == DOP_ETD1 || DOP == DOP_ETD2);
     auto kern = k_dir<R, DIR, DOP, DW>;
     const size_t sm = dir_smem_bytes(a.g.n, R, a.L, ETD ? 2 : 1, ETD ? 5 : 2, DW == DW_E);
-    kern<<<(unsigned)dir_tiles(a.g.n, a.L), a.threads > 0 ? a.threads : DLR_THREADS, sm, st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(kern, (unsigned)dir_tiles(a.g.n, a.L), a.threads > 0 ? a.threads : DLR_THREADS, sm, st, a);
 }

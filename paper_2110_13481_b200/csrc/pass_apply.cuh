@@ -45,6 +45,11 @@ __global__ void __launch_bounds__(DLR_APPLY_THREADS, 1) k_apply(const ApplyArgs 
     uint64_t* full = (uint64_t*)(mat + RR);                        // [S] (<= 8)
     __shared__ int s_last;
     const bool chol = a.ch.gsum != nullptr;
+    if (tid == 32) {
+        for (int s = 0; s < a.S; s++) mbar_init(full + s, 1);
+        mbar_fence_init();
+    }
+    pdl_wait();
     if (chol && a.ch.stage == 2 && a.ch.qrflag[0] != 0) return;   // third stage not needed
 
     const long long nchunks = a.N / C;
@@ -62,10 +67,6 @@ __global__ void __launch_bounds__(DLR_APPLY_THREADS, 1) k_apply(const ApplyArgs 
         if (pl < R)
             bulk_g2s(stage0 + (size_t)s * R * CS + (size_t)pl * CS, a.in + chunk_of(it) * C + (size_t)pl * a.N, col_bytes, full + s);
     };
-    if (tid == 32) {
-        for (int s = 0; s < S; s++) mbar_init(full + s, 1);
-        mbar_fence_init();
-    }
     __syncthreads();
     if (is_prod) {
         const int pre = nloc < S - 1 ? nloc : S - 1;
@@ -140,6 +141,7 @@ __global__ void __launch_bounds__(DLR_APPLY_THREADS, 1) k_apply(const ApplyArgs 
             }
         }
     }
+    pdl_trigger();
     if (is_prod) bulk_wait_read<0>();                               // every store has read its stage
     __syncthreads();
     if (want_gram) {
@@ -158,6 +160,5 @@ __global__ void __launch_bounds__(DLR_APPLY_THREADS, 1) k_apply(const ApplyArgs 
 
 template <int R, bool GRAM>
 inline cudaError_t launch_apply(const ApplyArgs& a, int ctas, cudaStream_t st) {
-    k_apply<R, GRAM><<<(unsigned)ctas, DLR_APPLY_THREADS, apply_smem_bytes(R, a.C, a.S), st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(k_apply<R, GRAM>, (unsigned)ctas, DLR_APPLY_THREADS, apply_smem_bytes(R, a.C, a.S), st, a);
 }

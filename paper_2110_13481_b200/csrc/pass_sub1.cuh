@@ -56,7 +56,8 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
     ZL zl;
     zl.L = NL; zl.lL = lNL; zl.ps = p.ps; zl.CP = wf_padded(n, p.ps) << lNL;
     double2* z = zbase + (size_t)grp * R * zl.CP;
-    wf_load_tables<LG>(tab, a.g.wtab);
+    wf_load_tables<LG>(tab, a.g.wtab);                      // written by dlr_create: may precede pdl_wait()
+    pdl_wait();
     const double invn = 1.0 / (double)n;
     for (int i = threadIdx.x; i < n * R; i += blockDim.x) {
         const int e = i / R, c = i - e * R;
@@ -145,6 +146,7 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
         wf_last<p.g[0]>(z, zl, R, lg, tab + p.toff[0], gp, st);
         gp.sync();                                            // the unit is free for the next one
     }
+    pdl_trigger();
     if (want_gram) {
         constexpr int P = R * (R + 1) / 2;
         __syncthreads();                                      // every unit is done: the buffers become reduction scratch
@@ -165,8 +167,7 @@ __global__ void __launch_bounds__(256, (R <= 10 ? 2 : 1)) k_sub1(const Sub1Args 
 template <int R, int LG>
 inline cudaError_t launch_sub1_lg(const Sub1Args& a, int groups, int ctas, cudaStream_t st) {
     const size_t sm = sub1_smem_bytes(1 << LG, R, a.NL, groups);
-    k_sub1<R, LG><<<(unsigned)ctas, groups * a.wpu * 32, sm, st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(k_sub1<R, LG>, (unsigned)ctas, groups * a.wpu * 32, sm, st, a);
 }
 
 template <int R>

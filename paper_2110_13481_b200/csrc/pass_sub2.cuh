@@ -37,7 +37,8 @@ __global__ void __launch_bounds__(256) k_sub2(const Sub2Args a) {
     zl.L = L; zl.lL = lL; zl.ps = p.ps; zl.CP = 0;
     const int ne = wf_padded(n, p.ps) << lL;
     double2* z = phs + n + (size_t)warp * ne;
-    wf_load_tables<LG>(tab, a.g.wtab);
+    wf_load_tables<LG>(tab, a.g.wtab);           // written by dlr_create: may precede pdl_wait()
+    pdl_wait();
     const double invn = 1.0 / (double)n;
     for (int e = threadIdx.x; e < n; e += blockDim.x) {
         const double2 f = a.ph[(size_t)e * a.R + c];
@@ -81,6 +82,7 @@ __global__ void __launch_bounds__(256) k_sub2(const Sub2Args a) {
             gp.sync();                              // the unit is free for the next one
         }
     }
+    pdl_trigger();
 }
 
 inline cudaError_t launch_sub2(const Sub2Args& a, int groups, int ctas_per_col, cudaStream_t st) {
@@ -88,15 +90,14 @@ inline cudaError_t launch_sub2(const Sub2Args& a, int groups, int ctas_per_col, 
     const int warps = groups * a.wpu;
     const dim3 grid((unsigned)ctas_per_col, (unsigned)a.R);
     switch (a.g.log2n) {
-        case 3: k_sub2<3><<<grid, warps * 32, sm, st>>>(a); break;
-        case 4: k_sub2<4><<<grid, warps * 32, sm, st>>>(a); break;
-        case 5: k_sub2<5><<<grid, warps * 32, sm, st>>>(a); break;
-        case 6: k_sub2<6><<<grid, warps * 32, sm, st>>>(a); break;
-        case 7: k_sub2<7><<<grid, warps * 32, sm, st>>>(a); break;
-        case 8: k_sub2<8><<<grid, warps * 32, sm, st>>>(a); break;
+        case 3: return dlr_launch(k_sub2<3>, grid, warps * 32, sm, st, a);
+        case 4: return dlr_launch(k_sub2<4>, grid, warps * 32, sm, st, a);
+        case 5: return dlr_launch(k_sub2<5>, grid, warps * 32, sm, st, a);
+        case 6: return dlr_launch(k_sub2<6>, grid, warps * 32, sm, st, a);
+        case 7: return dlr_launch(k_sub2<7>, grid, warps * 32, sm, st, a);
+        case 8: return dlr_launch(k_sub2<8>, grid, warps * 32, sm, st, a);
         default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
 }
 
 // resident CTAs per SM of the variant for this grid size (registers and shared memory)

@@ -29,6 +29,8 @@ __host__ __device__ constexpr int post_smem_doubles(int R) { return 21 * R * R +
 
 template <int R>
 __global__ void __launch_bounds__(DLR_POST_THREADS) k_post(const PostArgs a) {
+    pdl_wait();
+    pdl_trigger();
     constexpr int RR = R * R, P2 = R * (R - 1) / 2;
     extern __shared__ double psm[];
     const int tid = threadIdx.x, nth = blockDim.x;
@@ -210,8 +212,7 @@ __global__ void __launch_bounds__(DLR_POST_THREADS) k_post(const PostArgs a) {
 template <int R>
 inline cudaError_t launch_post(const PostArgs& a, cudaStream_t st) {
     static_assert(R * R <= DLR_POST_THREADS, "one thread per matrix entry");
-    k_post<R><<<a.do_tab ? 5 : 1, DLR_POST_THREADS, post_smem_doubles(R) * sizeof(double), st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(k_post<R>, a.do_tab ? 5 : 1, DLR_POST_THREADS, post_smem_doubles(R) * sizeof(double), st, a);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -237,6 +238,8 @@ __host__ __device__ constexpr size_t lpred_smem_bytes(int R, int n) { return (si
 
 template <int R>
 __global__ void __launch_bounds__(DLR_POST_THREADS) k_lpred_sums(const LpredArgs a) {
+    pdl_wait();
+    pdl_trigger();
     constexpr int RR = R * R;
     extern __shared__ double psm[];
     const int n = a.g.n, lg = a.g.log2n, tid = threadIdx.x, nth = blockDim.x;
@@ -319,6 +322,5 @@ __global__ void __launch_bounds__(DLR_POST_THREADS) k_lpred_sums(const LpredArgs
 
 template <int R>
 inline cudaError_t launch_lpred(const LpredArgs& a, cudaStream_t st) {
-    k_lpred_sums<R><<<1, DLR_POST_THREADS, lpred_smem_bytes(R, a.g.n), st>>>(a);
-    return cudaGetLastError();
+    return dlr_launch(k_lpred_sums<R>, 1, DLR_POST_THREADS, lpred_smem_bytes(R, a.g.n), st, a);
 }
