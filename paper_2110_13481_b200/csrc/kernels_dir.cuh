@@ -46,6 +46,11 @@ struct DirArgs {
     int threads;           // CTA size (0 = DLR_THREADS)
 };
 
+template <int DOP, int DW>
+__host__ __device__ inline bool dir_ereg(int n, int L, int threads) {
+    return (DOP == DOP_ETD1 || DOP == DOP_ETD2) && DW == DW_E && n * L <= threads;
+}
+
 __host__ __device__ inline int dir_tiles(int n, int L) { return (n * n / 2) / L; }     // same count for all directions
 
 // double2 elements of the tile region: at least the scratch of the cross-warp MMA reduction (64 doubles per warp)
@@ -209,7 +214,8 @@ DLR_CO_LOOP
 // its arguments through the stack)
 template <int R, int DIR, int DW>
 __device__ __forceinline__ void etd_realspace(double2* z, int LPZ, int pitems, int src_off, int dst_off, double scale,
-                                           const double* min_, const double* Q, const DirGeom gm, const double2* Et) {
+                                           const double* min_, const double* Q, const DirGeom gm, const double2* Et,
+                                           const bool wreg_on, const double2 (&wreg)[3]) {
     const int L = gm.L, lL = gm.lL;
     for (int w = threadIdx.x; w < pitems; w += blockDim.x) {
         const int l = w & (L - 1), e = w >> lL;
@@ -222,8 +228,8 @@ __device__ __forceinline__ void etd_realspace(double2* z, int LPZ, int pitems, i
 #pragma unroll
             for (int c = 0; c < R; c++) x[c] = p[src_off + c * L];       // this thread's own stores
         }
-        double2 w0, w1, w2;
-        dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
+        double2 w0 = wreg[0], w1 = wreg[1], w2 = wreg[2];                // the thread's own point (field weights in registers)
+        if (!wreg_on) dir_weights<DIR, DW>(gm, Et, e, l, w0, w1, w2);
         dir_nonlin<R>(x, p + dst_off, L, Q, w0, w1, w2);                 // x is fully in registers: dst may be src
     }
     __syncthreads();
@@ -272,6 +278,11 @@ k_dir(const DirArgs a) {
     pdl_wait();
     const size_t N2 = (size_t)(a.g.N >> 1);
     const double invn = 1.0 / (double)n;
+    // Field weights of the third sub-flow: with at most one tile point per thread they stay in registers for both
+    // evaluations of the real-space term and the tile needs no field rows in shared memory (64^3, r = 10: 103 -> 91 KB per
+    // CTA, which leaves the two resident CTAs an L1 large enough for the e^z / phi tables they read in Fourier space)
+    const bool ereg = dir_ereg<DOP, DW>(n, L, (int)nth);
+    double2 wreg[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
 
     // Passes without point-wise work across the columns before the transform (direction-2 sub-flow, Parseval-only
     // coefficient passes) feed the first FFT group straight from global memory (and the sub-flow writes its last inverse
@@ -304,7 +315,13 @@ k_dir(const DirArgs a) {
                 cp_async16(z + (size_t)e * LPZ + c * L + l, in2 + (size_t)c * N2 + dir_index<DIR>(gm, e, l));
             }
         }
-        if (DW == DW_E) {
+        if (DW == DW_E && ereg) {
+            if (tid < (n << lL)) {
+                const int l = tid & (L - 1), e = tid >> lL;
+#pragma unroll
+                for (int d = 0; d < 3; d++) wreg[d] = ((const double2*)(a.E + (size_t)d * a.g.N))[dir_index<DIR>(gm, e, l)];
+            }
+        } else if (DW == DW_E) {
             for (int d = 0; d < 3; d++) {
                 const double2* e2 = (const double2*)(a.E + (size_t)d * a.g.N);
                 double2* Ed = Et + (size_t)d * n * L;
@@ -443,7 +460,7 @@ k_dir(const DirArgs a) {
         // -------------------------------------------------------------- third sub-flow, exponential Runge-Kutta
         const double* Q = mats + 2 * MS;
         // m = A Min,  g0 = N'(m)
-        etd_realspace<R, DIR, DW>(z, LPZ, pitems, 0, nl, 1.0, a.min_ != nullptr ? mats : nullptr, Q, gm, Et);
+        etd_realspace<R, DIR, DW>(z, LPZ, pitems, 0, nl, 1.0, a.min_ != nullptr ? mats : nullptr, Q, gm, Et, ereg, wreg);
         // Fourier-space stages fused into the middle FFT group (fft_mid2): the spectra of m and g0 never make a round
         // trip through shared memory.  a = e^z M^ + t phi1 G0^  (stage-1 state);  ETD2RK keeps  e^z M^ + t (phi1 - phi2) G0^
         // in buffer A (spectral) and adds t phi2 G1^ to it after the second evaluation of the real-space term.
@@ -463,7 +480,7 @@ k_dir(const DirArgs a) {
                 bv = ah;                                      // inverse-transformed for N'(a)
             });
             fft_lines_c<true>(z + nl, LPZ, nl, lg, true);
-            etd_realspace<R, DIR, DW>(z, LPZ, pitems, nl, nl, invn, nullptr, Q, gm, Et);      // g1 = N'(a), in place
+            etd_realspace<R, DIR, DW>(z, LPZ, pitems, nl, nl, invn, nullptr, Q, gm, Et, ereg, wreg);      // g1 = N'(a), in place
             fft_lines_c<false>(z + nl, LPZ, nl, lg, true);
             fft_mid2<false, true, true, false, true, false>(z, nl, LPZ, nl, lg, [&](double2& av, double2& bv, int e, int line) {
                 av = cadd(av, cmul(bv, __ldg(a.f2b + (size_t)e * R + (line >> lL))));
@@ -546,6 +563,7 @@ template <int R, int DIR, int DOP, int DW>
 inline cudaError_t launch_dir(const DirArgs& a, cudaStream_t st) {
     constexpr bool ETD = (DOP == DOP_ETD1 || DOP == DOP_ETD2);
     auto kern = k_dir<R, DIR, DOP, DW>;
-    const size_t sm = dir_smem_bytes(a.g.n, R, a.L, ETD ? 2 : 1, ETD ? 5 : 2, DW == DW_E);
-    return dlr_launch(kern, (unsigned)dir_tiles(a.g.n, a.L), a.threads > 0 ? a.threads : DLR_THREADS, sm, st, a);
+    const int threads = a.threads > 0 ? a.threads : DLR_THREADS;
+    const size_t sm = dir_smem_bytes(a.g.n, R, a.L, ETD ? 2 : 1, ETD ? 5 : 2, DW == DW_E && !dir_ereg<DOP, DW>(a.g.n, a.L, threads));
+    return dlr_launch(kern, (unsigned)dir_tiles(a.g.n, a.L), threads, sm, st, a);
 }
