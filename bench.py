@@ -300,24 +300,42 @@ def main():
         tpath = os.path.join(ROOT, "profiles", "r02_traffic.json")
         if os.path.exists(tpath):
             traffic = json.load(open(tpath)).get(top["kernel"].split(" ")[0])
+        # which roofline binds a kernel: the larger of its two floors, algorithmic bytes / HBM peak and algorithmic
+        # fp64 flops / fp64 peak (plain ALUs: the fp64 tensor path has the same peak on B200)
+        for k in kernels:
+            t_hbm = k["algorithmic_bytes_per_launch"] / (peak * 1e9)
+            t_alu = k["algorithmic_flops_per_launch"] / (FP64_TFLOPS * 1e12)
+            k["bound"] = "alu" if t_alu > t_hbm else "hbm"
+            k["frac"] = max(t_hbm, t_alu) / (k["avg_us"] * 1e-6)
+            k["frac_hbm"], k["frac_alu"] = k["gbs"] / peak, k["tflops"] / FP64_TFLOPS
+        flops_step = sum(k["algorithmic_flops_per_launch"] * k["launches_per_step"] for k in kernels)
+        alu = top["bound"] == "alu"
         roofline = {
-            "bound": "hbm", "kernel": top["kernel"], "achieved": top["gbs"], "peak": peak, "unit": "GB/s",
-            "frac": top["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
-            "algorithmic_bytes_per_launch": top["algorithmic_bytes_per_launch"], "avg_launch_us": top["avg_us"],
+            "bound": top["bound"], "kernel": top["kernel"],
+            "achieved": top["tflops"] if alu else top["gbs"], "peak": FP64_TFLOPS if alu else peak,
+            "unit": "TFLOP/s" if alu else "GB/s", "frac": top["frac"], "traffic": traffic,
+            "peak_source": ("fp64 vector peak derived in DESIGN.md section 6: 148 SMs x 64 fp64 lanes x 2 x 1.965 GHz = 37.2 "
+                            "TFLOP/s, a DFMA-only kernel measured 36.8 on this pool (profiles/r02_peaks.md); HBM: " + peak_src)
+                           if alu else peak_src,
+            "algorithmic_bytes_per_launch": top["algorithmic_bytes_per_launch"],
+            "algorithmic_flops_per_launch": top["algorithmic_flops_per_launch"], "avg_launch_us": top["avg_us"],
             "launches_per_step": top["launches_per_step"], "share_of_step": top["share_of_step"],
-            "alu": {"achieved": top["tflops"], "peak": FP64_TFLOPS, "unit": "TFLOP/s", "frac": top["tflops"] / FP64_TFLOPS,
-                    "what": "plain fp64 ALUs: algorithmic flops of the launch (DESIGN.md section 6) / its duration; peak = "
-                            "148 SMs x 64 fp64 lanes x 2 x 1.965 GHz = 37.2, measured 36.8 (profiles/r02_peaks.md)"},
+            "hbm": {"achieved": top["gbs"], "peak": peak, "unit": "GB/s", "frac": top["gbs"] / peak, "peak_source": peak_src},
+            "alu": {"achieved": top["tflops"], "peak": FP64_TFLOPS, "unit": "TFLOP/s", "frac": top["tflops"] / FP64_TFLOPS},
             "note": "dominant kernel family of the step by device time; duration = CUDA events after every launch on "
                     "the context's stream (dlr_set_profiling(ctx, 2), 5 steps, median) right after the timed region; "
                     "traffic = DRAM bytes per launch from the ncu --set full capture of this build in profiles/ (cold "
-                    "cache). bound = hbm is the roofline the metric asks for. As measured (profiles/r02_profile_cfg3.md) no "
-                    "pass kernel is HBM-bound at this shape: DRAM traffic = algorithmic bytes, the 21 MB factor is L2-resident, "
-                    "and the kernels are LATENCY- and ISSUE-bound (warps active ~22 %, issue slots 27-35 %, fp64 pipe 22-27 %, "
-                    "no pipe above 50 %): the third sub-flow executes 26 M warp instructions per launch (issue floor 22 us, "
-                    "fp64 floor 18 us) in 11 barrier-separated phases of one tile",
+                    "cache). bound = the larger of the kernel's two floors (algorithmic bytes / measured HBM copy peak, "
+                    "algorithmic fp64 flops / fp64 peak): the third sub-flow has 13 flop per byte against a machine balance "
+                    "of 5.6, so the fp64 ALUs bound it; both fractions are in hbm/alu. As measured (profiles/) no pass kernel "
+                    "is HBM-bound at this shape (DRAM traffic = algorithmic bytes, the 21 MB factor is L2-resident) and none "
+                    "reaches its ALU floor: they are latency-, barrier- and instruction-fetch-bound (warps active ~22 %, "
+                    "issue slots ~33 %, fp64 pipe ~30 %)",
             "step": {"algorithmic_bytes_per_step": bytes_step, "achieved": achieved, "frac": achieved / peak,
-                     "what": "all factor-sized passes of one step (DESIGN.md section 6) / CUDA-event time of the step"},
+                     "alu_tflops": flops_step / (ms_step * 1e-3) / 1e12,
+                     "alu_frac": flops_step / (ms_step * 1e-3) / 1e12 / FP64_TFLOPS,
+                     "what": "all factor-sized passes of one step (DESIGN.md section 6) / CUDA-event time of the step; "
+                             "alu_*: the algorithmic fp64 flops of the pass kernels of one step / the same time"},
             "kernels": kernels,
         }
         out = {

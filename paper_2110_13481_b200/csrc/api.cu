@@ -489,7 +489,8 @@ void setup_sub2(dlr_ctx* c, const HostGrid& hg, Sub2Cfg& sc) {
     const int n = hg.g.n, M = n / 2;
     sc.L = n <= 64 ? std::min(M, 8) : 4;
     sc.wpu = n >= 256 ? 2 : 1;
-    sc.groups = n >= 256 ? 2 : 4;                 // measured at 256^3, r = 20: 2123 -> 1956 us per pass with two 2-warp groups
+    sc.groups = n >= 256 ? 2 : (n <= 64 ? 5 : 4); // measured at 256^3, r = 20: 2123 -> 1956 us per pass with two 2-warp groups;
+                                                  // at 64^3, r = 10 (us per pass): 2 groups 19.0, 3: 15.5, 4: 15.6, 5: 15.1, 8: 17.0
     { const int l = tune("s2l", 0); if (is_pow2(l) && l <= M) sc.L = l; }
     { const int w = tune("s2w", 0); if (w >= 1 && w <= 8) sc.groups = w; }
     { const int w = tune("s2u", 0); if (w == 1 || w == 2 || w == 4) sc.wpu = w; }
@@ -524,9 +525,20 @@ void setup_sub1(dlr_ctx* c, const HostGrid& hg, Sub1Cfg& sc) {
     while (sc.groups > 1 && sub1_smem_bytes(n, R, sc.NL, sc.groups) > target) sc.groups--;
     if (sub1_smem_bytes(n, R, sc.NL, sc.groups) > SMEM_MAX - 1024) sc.use = 0;
     if (!sc.use) return;
-    const int per_sm = c->ops->sub1_occ(hg.g.log2n, sc.groups * sc.wpu * 32, sub1_smem_bytes(n, R, sc.NL, sc.groups));
     const int units = (n * n / 2) / sc.NL;
-    sc.ctas = std::max(1, std::min(c->nsm * per_sm, (units + sc.groups - 1) / sc.groups));
+    // Every warp (group) owns whole units and all warps of the single wave run in step, so the pass lasts as long as the
+    // SM with the most units: one group fewer per CTA can spread the units evenly (64^3, r = 10: 2048 units as 256 CTAs of
+    // 8 warps put 16 on 108 SMs and 8 on the others; 293 CTAs of 7 warps put 14 on each: 30.1 -> 28.1 us per pass)
+    const auto plan = [&](int g, int& ctas) {
+        const int per_sm = c->ops->sub1_occ(hg.g.log2n, g * sc.wpu * 32, sub1_smem_bytes(n, R, sc.NL, g));
+        ctas = std::max(1, std::min(c->nsm * per_sm, (units + g - 1) / g));
+        const int upw = (units + ctas * g - 1) / (ctas * g);
+        return ((ctas + c->nsm - 1) / c->nsm) * g * upw;           // units of the busiest SM
+    };
+    int ctas_a = 1, ctas_b = 1;
+    const int cost_a = plan(sc.groups, ctas_a);
+    sc.ctas = ctas_a;
+    if (sc.groups > 2 && tune("s1w", 0) == 0 && plan(sc.groups - 1, ctas_b) < cost_a) { sc.groups--; sc.ctas = ctas_b; }
 }
 cudaError_t run_sub1(dlr_ctx* c, const HostGrid& hg, const DirArgs& d) {
     const Sub1Cfg& sc = (&hg == &c->gx) ? c->s1x : c->s1v;

@@ -203,12 +203,14 @@ __host__ __device__ inline int dlr_groups(int nblocks) { return (nblocks + DLR_G
 __device__ __forceinline__ void group_prereduce(const double* rows, int nvals, unsigned* counters, double* rows2,
                                                 double* final_row = nullptr) {
     __shared__ int s_last;
-    __threadfence();
-    __syncthreads();
+    __syncthreads();                                           // the partial row of this CTA is written (CTA scope) ...
     const int grp = (int)blockIdx.x / DLR_GRP, first = grp * DLR_GRP;
     const int cnt = min(DLR_GRP, (int)gridDim.x - first);
-    if (threadIdx.x == 0) s_last = (atomicInc(counters + grp, (unsigned)(cnt - 1)) == (unsigned)(cnt - 1));
-    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();                                       // ... and ordered device-wide before the counter moves: ONE
+        s_last = (atomicInc(counters + grp, (unsigned)(cnt - 1)) == (unsigned)(cnt - 1));   // fence per CTA (cumulative
+    }                                                          // over the barrier), not one per thread (ncu: 7-14 % of
+    __syncthreads();                                           // the stall samples of the coefficient passes were membar)
     if (!s_last) return;
     __threadfence();
     for (int v = threadIdx.x; v < nvals; v += blockDim.x) {
@@ -219,10 +221,11 @@ __device__ __forceinline__ void group_prereduce(const double* rows, int nvals, u
     }
     if (final_row == nullptr) return;
     const int ngrp = dlr_groups((int)gridDim.x);
-    __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0)
+    if (threadIdx.x == 0) {
+        __threadfence();
         s_last = (atomicInc(counters + DLR_CNT_STRIDE - 1, (unsigned)(ngrp - 1)) == (unsigned)(ngrp - 1));
+    }
     __syncthreads();
     if (!s_last) return;
     __threadfence();
