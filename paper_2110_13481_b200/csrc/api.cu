@@ -46,6 +46,7 @@ struct HostGrid {
     int thr1, thr2, thr3; // CTA sizes of the three pass families
     int Lx, Le, Lc;       // directional passes: packed lines per column for EXACT, ETD and COEFF tiles
     int thrx, thre, thrc; // CTA sizes of the EXACT, ETD and COEFF directional passes
+    int Lc2, thrc2;       // the Parseval-only coefficient passes (directions 2, 3)
     int thrx2;            // CTA size of the direction-2 sub-flow (register-light: up to 512 threads)
 };
 
@@ -262,7 +263,7 @@ size_t carve(dlr_ctx* c, char* base) {
     for (const HostGrid* hg : {&c->gx, &c->gv}) {
         size_t b1 = (size_t)hg->g.n * hg->g.n / hg->T1;
         size_t bd = (size_t)dir_tiles(hg->g.n, 1);            // directional tiles at L = 1 (the most there can be)
-        bd = std::max(bd / hg->Lx, std::max(bd / hg->Le, bd / hg->Lc));
+        bd = std::max(std::max(bd / hg->Lx, bd / hg->Lc2), std::max(bd / hg->Le, bd / hg->Lc));
         blocks = std::max(blocks, std::max(b1, bd));
         blocks = std::max(blocks, std::min((size_t)dir_tiles(hg->g.n, 1), (size_t)2048));   // persistent grids (pass_sub1.cuh)
     }
@@ -367,6 +368,11 @@ void setup_grid(HostGrid& hg, int n, double lo, double hi, int R) {
     if (is_pow2(lx) && lx <= n / 2 && dir_smem_bytes(n, R, lx, 1, 2, false) <= SMEM_MAX) hg.Lx = lx;
     if (is_pow2(le) && le <= n / 2 && dir_smem_bytes(n, R, le, 2, 5, true) <= SMEM_MAX) hg.Le = le;
     if (is_pow2(lc) && lc <= n / 2 && dir_smem_bytes(n, R, lc, 1, 2, true) <= SMEM_MAX) hg.Lc = lc;
+    // Parseval-only passes (no weighted Gram): at 64^3, r = 10 half-size tiles with 192 threads, three CTAs per SM, read the
+    // factor in 22.6 / 20.6 us (directions 2 / 3) against 23.7 / 22.6 with the tiles of the first pass (which wants them
+    // large: 42.6 us at L = 8, 52.9 at L = 4)
+    hg.Lc2 = hg.Lc; hg.thrc2 = hg.thrc;
+    if (n == 64 && R <= 10 && hg.Lc == 8 && tune("lc", 0) == 0 && tune("thrc", 0) == 0) { hg.Lc2 = 4; hg.thrc2 = 192; }
     if (hg.thrx2 == 0) {
         // the direction-2 sub-flow is register-light (up to 512 threads per CTA): 320 threads when the butterfly items of
         // an FFT group (n/8 per line) then divide evenly, e.g. 640 items at n = 64, r = 10, 8 lines per column
@@ -571,6 +577,7 @@ void coeffs(dlr_ctx* c, const HostGrid& hg, const double* A, int kind, double* M
     CK(cudaEventRecord(c->ev_join, c->side));
     c->count_launches -= 3;                         // the three event calls above are not kernel launches
     a.gram = nullptr; a.E = nullptr;
+    a.L = hg.Lc2; a.threads = hg.thrc2;
     a.pgram = c->partialP[1]; a.pgram2 = c->pgram2[1]; a.pgramF = c->pgramF[1];
     CK(c->ops->dir[VD_COEFF2](a, c->st));
     a.pgram = c->partialP[2]; a.pgram2 = c->pgram2[2]; a.pgramF = c->pgramF[2];

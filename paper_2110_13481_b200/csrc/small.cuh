@@ -62,6 +62,9 @@ __device__ __forceinline__ void cta_reduce_rows(const double* __restrict__ parti
 //   buffer (two barriers per round instead of a serial chain of R(R-1)/2 rotations per sweep).
 // partial: [nblocks][3P (+R)], entry e of direction d at d*P + e, column sums at 3P + c.
 #define DLR_EIG_THREADS 256
+#ifndef DLR_EIG_TOL2
+#define DLR_EIG_TOL2 1e-20
+#endif
 __global__ void __launch_bounds__(DLR_EIG_THREADS)
 k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double h3, double* M1, double* colsum,
              double* Tout, double* lam, int warm, int* status) {
@@ -176,7 +179,10 @@ k_coeff1_eig(const double* partial, int nblocks, int R, int with_colsum, double 
             s_off2 = o;
         }
         __syncthreads();
-        if (s_off2 <= 1e-32 * nrm2) { converged = true; break; }   // off-diagonal norm met in this sweep <= 1e-16 ||A||_F
+        // Converged when the off-diagonal norm MET in this sweep (before its rotations) is <= 1e-10 ||A||_F: cyclic Jacobi
+        // converges quadratically, so after the rotations of this sweep it is at rounding level (<= ~1e-20 ||A||_F^2 / gap);
+        // waiting until a sweep meets <= 1e-16 ||A||_F costs one more full sweep for nothing
+        if (s_off2 <= DLR_EIG_TOL2 * nrm2) { converged = true; break; }
     }
     if (!converged && tid == 0) atomicAdd(status + 3, 1);      // sweep cap hit: reported as dlr_moments_t.eig_unconverged
     if (warm) {
